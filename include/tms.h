@@ -1,0 +1,152 @@
+/*
+ * tms.h -- C ABI of the B200-native MaxSim scoring library (libtms.so).
+ *
+ * Implements the data-parallel hot path of "TileMaxSim" (arXiv 2606.26439; the paper text is cited
+ * below as P:L<line> of PAPER.md):
+ *   - tms_maxsim        : fused multi-query MaxSim over a packed token-major document store,
+ *                         including the dimension-tiled form for d > 128 (Eq. 1;
+ *                         P:L182-204 Alg. 3).
+ *   - tms_pq_build_lut  : product-quantisation distance table, Eq. 8.
+ *   - tms_pq_maxsim     : fused lookup + max + sum over uint8 PQ codes, Eq. 9.
+ *   - tms_maxsim_host / tms_pq_maxsim_host : the same scoring from HOST buffers, the document store
+ *                         streamed through a caller-provided device workspace.
+ *
+ * Conventions, unless a function says otherwise:
+ *   - "device" pointers are CUDA device memory on the current device, owned by the caller.  The
+ *     library never allocates or frees device memory; scratch comes through `workspace`.
+ *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream) and return without synchronising the host.
+ *   - The return value is a tms_status describing host-side argument / launch errors.  There are no
+ *     exceptions, no errno, no logging.  Data errors the host cannot see without a sync (for
+ *     instance non-monotone `offsets`) are undefined behaviour.
+ *   - `scores` is fully overwritten for all Q*B entries; it is never accumulated into and needs no
+ *     initialisation.
+ *   - Inputs must be finite.  An empty document (offsets[b+1] == offsets[b]) scores -INFINITY, the
+ *     literal outcome of "m <- -inf" in Alg. 3 line 4.
+ *   - Similarity is the raw dot product of Eq. 1; normalisation is the caller's business.
+ *   - There is no CPU fallback: on a machine without a usable sm_100 device the compute entry points
+ *     return TMS_ERR_UNSUPPORTED or TMS_ERR_CUDA.
+ */
+#ifndef TMS_H_
+#define TMS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TMS_OK = 0,
+    TMS_ERR_INVALID_ARG = 1, /* NULL pointer, non-positive size, inconsistent sizes            */
+    TMS_ERR_UNSUPPORTED = 2, /* shape / dtype / device outside what this build implements      */
+    TMS_ERR_ALIGNMENT = 3,   /* a pointer or row pitch is not 16-byte aligned                  */
+    TMS_ERR_WORKSPACE = 4,   /* workspace is NULL or smaller than the *_workspace_bytes() size  */
+    TMS_ERR_CUDA = 5         /* a CUDA runtime / driver call failed (launch, copy, attribute)  */
+} tms_status;
+
+/* Storage dtype of query and document embeddings.  Arithmetic: products of the stored values,
+ * accumulated in fp32 ("FP16 embeddings with FP32 accumulation"). */
+typedef enum { TMS_DTYPE_F32 = 0, TMS_DTYPE_F16 = 1, TMS_DTYPE_BF16 = 2 } tms_dtype;
+
+/* Kernel selection for tms_maxsim_variant / tms_pq_maxsim_variant (tests, benches, ablations). */
+typedef enum {
+    TMS_VARIANT_AUTO = 0,     /* what tms_maxsim / tms_pq_maxsim pick                                  */
+    TMS_VARIANT_SIMT = 1,     /* CUDA-core tiled kernel: any dtype, any d, any Nq (the general path)   */
+    TMS_VARIANT_TCGEN05 = 2,  /* TMA + tcgen05 tensor-core kernel (sm_100a), dimension-tiled for d>128 */
+    TMS_VARIANT_PQ_SMEM = 3   /* PQ: LUT slices resident in shared memory                              */
+} tms_variant;
+
+/*
+ * Dense MaxSim (Eq. 1):
+ *     scores[q*B + b] = sum_{i<Nq}  max_{t in [offsets[b], offsets[b+1])}  <queries[q,i,:], docs[t,:]>
+ *
+ * queries       device, [Q, Nq, d] row-major, `dtype`, 16-byte aligned.
+ * docs          device, packed token-major store [total_tokens, d] row-major, `dtype`, 16-byte
+ *               aligned base; the row pitch d*sizeof(dtype) must be a multiple of 16 bytes.
+ * offsets       device, int64 [B+1]; offsets[0] = 0, non-decreasing, offsets[B] = total_tokens.
+ * total_tokens  = offsets[B]; passed by value so the host never reads device memory.
+ * scores        device, fp32 [Q, B] row-major, overwritten.
+ * workspace     device scratch of at least tms_maxsim_workspace_bytes(...) bytes; may be NULL when
+ *               that size is 0.
+ * Every document embedding is read from HBM once per group of up to 256 query rows (Q*Nq, with Nq
+ * rounded up to a power of two); no similarity matrix is written to memory (Eq. 7).
+ * d > 128 accumulates partial dot products over dimension chunks before the max is taken.
+ */
+int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
+               int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace, size_t workspace_bytes,
+               void* stream);
+
+/* Same as tms_maxsim with an explicit kernel choice.  A variant that cannot run the given shape
+ * returns TMS_ERR_UNSUPPORTED instead of silently switching. */
+int tms_maxsim_variant(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets,
+                       int64_t B, int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace,
+                       size_t workspace_bytes, void* stream, tms_variant variant);
+
+size_t tms_maxsim_workspace_bytes(int Q, int Nq, int d, int64_t B, tms_dtype dtype);
+
+/*
+ * PQ distance table (Eq. 8):
+ *     lut[q,i,m,k] = sum_{s<d/M} queries[q,i,m*(d/M)+s] * codebooks[m,k,s]      (fp32 FMA, s ascending)
+ * queries    device, [Q, Nq, d], `q_dtype`.      codebooks  device, fp32 [M, K, d/M].
+ * lut        device, fp32 [Q, Nq, M, K], overwritten.     Requires d % M == 0 and 1 <= K <= 256.
+ */
+int tms_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                     int K, float* lut, void* stream);
+
+/*
+ * Fused PQ scoring (Eq. 9; phase 2 of P:L270):
+ *     scores[q*B + b] = sum_{i<Nq}  max_{t in doc b}  sum_{m<M} lut[q,i,m,codes[t,m]]
+ * lut      device, fp32 [Q, Nq, M, K] as written by tms_pq_build_lut.
+ * codes    device, uint8 [total_tokens, M] row-major, 16-byte aligned base; values < K.
+ * The decompressed vectors are never materialised.  The sum over m is fp32 in a fixed, kernel-defined
+ * order (run-to-run reproducible).
+ * workspace  device scratch of at least tms_pq_workspace_bytes(...) bytes (the re-laid-out table).
+ */
+int tms_pq_maxsim(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes, const int64_t* offsets,
+                  int64_t B, int64_t total_tokens, float* scores, void* workspace, size_t workspace_bytes,
+                  void* stream);
+
+int tms_pq_maxsim_variant(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes,
+                          const int64_t* offsets, int64_t B, int64_t total_tokens, float* scores, void* workspace,
+                          size_t workspace_bytes, void* stream, tms_variant variant);
+
+size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B);
+
+/*
+ * Host-buffer entry points: identical results, but `queries`, `docs` / `codes`, `offsets`, `codebooks` and
+ * `scores` are HOST pointers (pinned memory makes the copies asynchronous and fast).  The document store
+ * is streamed through `dev_workspace` in document-aligned chunks; the host->device copy of chunk n+1 runs
+ * on an internal copy stream while chunk n is scored on `stream`; each chunk's scores return with one
+ * strided device->host copy.  Unlike the device entry points these calls validate `offsets` (host memory)
+ * and return only after the scores have landed in `scores` (they synchronise `stream`).
+ *
+ * dev_workspace   device memory, at least *_host_workspace_min_bytes(..., max_doc_tokens) bytes where
+ *                 max_doc_tokens is the longest document; a larger workspace means fewer, larger chunks.
+ *                 TMS_ERR_WORKSPACE if a single document does not fit in half of what remains after the
+ *                 query (and, for PQ, table) staging area.
+ * tms_pq_maxsim_host builds the distance table on the device from host `queries` and `codebooks` first.
+ */
+int tms_maxsim_host(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
+                    int64_t total_tokens, tms_dtype dtype, float* scores, void* dev_workspace,
+                    size_t dev_workspace_bytes, void* stream);
+
+int tms_pq_maxsim_host(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                       int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
+                       float* scores, void* dev_workspace, size_t dev_workspace_bytes, void* stream);
+
+size_t tms_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype dtype, int64_t max_doc_tokens);
+size_t tms_pq_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype q_dtype, int M, int K,
+                                              int64_t max_doc_tokens);
+
+/* Number of kernels this library has launched in this process since load (all entry points). */
+uint64_t tms_launch_count(void);
+
+const char* tms_status_string(int status);
+int tms_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TMS_H_ */

@@ -1,0 +1,169 @@
+// api.cu -- the C ABI of libtms.so (include/tms.h): argument validation and kernel dispatch only.
+#include <atomic>
+#include <mutex>
+
+#include "tms_internal.h"
+
+namespace tms {
+
+static std::atomic<uint64_t> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+
+const DeviceInfo* device_info() {
+    static std::mutex mu;
+    static DeviceInfo cache[64];
+    static bool have[64] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!have[dev]) {
+        DeviceInfo di;
+        di.device = dev;
+        if (cudaDeviceGetAttribute(&di.cc_major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&di.cc_minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&di.num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&di.max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        cache[dev] = di;
+        have[dev] = true;
+    }
+    return &cache[dev];
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_dense(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
+                       int64_t T, tms_dtype dtype, float* scores) {
+    if (Q <= 0 || Nq <= 0 || d <= 0 || B < 0 || T < 0) return TMS_ERR_INVALID_ARG;
+    if (dtype != TMS_DTYPE_F32 && dtype != TMS_DTYPE_F16 && dtype != TMS_DTYPE_BF16) return TMS_ERR_INVALID_ARG;
+    if (!queries || !offsets || (B > 0 && !scores) || (T > 0 && !docs)) return TMS_ERR_INVALID_ARG;
+    if ((int64_t)Q * Nq > (1 << 20) || (int64_t)Q * B < 0) return TMS_ERR_UNSUPPORTED;
+    if (((size_t)d * dtype_size(dtype)) % 16 != 0) return TMS_ERR_UNSUPPORTED;  // row pitch (a1)
+    if (!aligned16(queries) || !aligned16(docs) || (reinterpret_cast<uintptr_t>(offsets) & 7u) ||
+        (reinterpret_cast<uintptr_t>(scores) & 3u))
+        return TMS_ERR_ALIGNMENT;
+    return TMS_OK;
+}
+
+static int dense_dispatch(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets,
+                          int64_t B, int64_t T, tms_dtype dtype, float* scores, void* stream, tms_variant variant) {
+    int st = check_dense(queries, Q, Nq, d, docs, offsets, B, T, dtype, scores);
+    if (st != TMS_OK) return st;
+    if (!device_info()) return TMS_ERR_CUDA;
+    if (B == 0) return TMS_OK;
+    DenseArgs a{queries, Q, Nq, d, docs, offsets, B, T, dtype, scores, static_cast<cudaStream_t>(stream)};
+    switch (variant) {
+        case TMS_VARIANT_AUTO: return dense_tc_supports(a) ? launch_dense_tc(a) : launch_dense_simt(a);
+        case TMS_VARIANT_SIMT: return launch_dense_simt(a);
+        case TMS_VARIANT_TCGEN05: return dense_tc_supports(a) ? launch_dense_tc(a) : TMS_ERR_UNSUPPORTED;
+        default: return TMS_ERR_INVALID_ARG;
+    }
+}
+
+static int check_pq(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes, const int64_t* offsets,
+                    int64_t B, int64_t T, float* scores) {
+    if (Q <= 0 || Nq <= 0 || M <= 0 || K <= 0 || B < 0 || T < 0) return TMS_ERR_INVALID_ARG;
+    if (!lut || !offsets || (B > 0 && !scores) || (T > 0 && !codes)) return TMS_ERR_INVALID_ARG;
+    if (K > 256 || M > 256 || (int64_t)Q * Nq > (1 << 20)) return TMS_ERR_UNSUPPORTED;
+    if (!aligned16(lut) || !aligned16(codes) || (reinterpret_cast<uintptr_t>(offsets) & 7u) ||
+        (reinterpret_cast<uintptr_t>(scores) & 3u))
+        return TMS_ERR_ALIGNMENT;
+    return TMS_OK;
+}
+
+static int pq_dispatch(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes, const int64_t* offsets,
+                       int64_t B, int64_t T, float* scores, void* workspace, size_t workspace_bytes, void* stream,
+                       tms_variant variant) {
+    int st = check_pq(lut, Q, Nq, M, K, codes, offsets, B, T, scores);
+    if (st != TMS_OK) return st;
+    if (!device_info()) return TMS_ERR_CUDA;
+    if (B == 0) return TMS_OK;
+    PqArgs a{lut, Q, Nq, M, K, codes, offsets, B, T, scores, static_cast<cudaStream_t>(stream)};
+    const bool smem_ok = pq_smem_supports(a);
+    if (variant == TMS_VARIANT_SIMT || (variant == TMS_VARIANT_AUTO && !smem_ok)) return launch_pq_simt(a);
+    if (variant != TMS_VARIANT_AUTO && variant != TMS_VARIANT_PQ_SMEM) return TMS_ERR_INVALID_ARG;
+    if (!smem_ok) return TMS_ERR_UNSUPPORTED;
+    if (!workspace || workspace_bytes < pq_smem_workspace_bytes(Q, Nq) || !aligned16(workspace))
+        return TMS_ERR_WORKSPACE;
+    return launch_pq_smem(a, workspace);
+}
+
+}  // namespace tms
+
+using namespace tms;
+
+extern "C" {
+
+int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
+               int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace, size_t workspace_bytes,
+               void* stream) {
+    (void)workspace;
+    (void)workspace_bytes;
+    return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, stream, TMS_VARIANT_AUTO);
+}
+
+int tms_maxsim_variant(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets,
+                       int64_t B, int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace,
+                       size_t workspace_bytes, void* stream, tms_variant variant) {
+    (void)workspace;
+    (void)workspace_bytes;
+    return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, stream, variant);
+}
+
+size_t tms_maxsim_workspace_bytes(int Q, int Nq, int d, int64_t B, tms_dtype dtype) {
+    (void)Q; (void)Nq; (void)d; (void)B; (void)dtype;
+    return 0;  // the dense path needs no scratch: no partial results ever leave the SM
+}
+
+int tms_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                     int K, float* lut, void* stream) {
+    if (Q <= 0 || Nq <= 0 || d <= 0 || M <= 0 || K <= 0) return TMS_ERR_INVALID_ARG;
+    if (!queries || !codebooks || !lut) return TMS_ERR_INVALID_ARG;
+    if (q_dtype != TMS_DTYPE_F32 && q_dtype != TMS_DTYPE_F16 && q_dtype != TMS_DTYPE_BF16) return TMS_ERR_INVALID_ARG;
+    if (d % M != 0 || K > 256 || M > 65535) return TMS_ERR_UNSUPPORTED;
+    if (!device_info()) return TMS_ERR_CUDA;
+    return launch_pq_build_lut(queries, Q, Nq, d, q_dtype, codebooks, M, K, lut, static_cast<cudaStream_t>(stream));
+}
+
+int tms_pq_maxsim(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes, const int64_t* offsets,
+                  int64_t B, int64_t total_tokens, float* scores, void* workspace, size_t workspace_bytes,
+                  void* stream) {
+    return pq_dispatch(lut, Q, Nq, M, K, codes, offsets, B, total_tokens, scores, workspace, workspace_bytes, stream,
+                       TMS_VARIANT_AUTO);
+}
+
+int tms_pq_maxsim_variant(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes,
+                          const int64_t* offsets, int64_t B, int64_t total_tokens, float* scores, void* workspace,
+                          size_t workspace_bytes, void* stream, tms_variant variant) {
+    return pq_dispatch(lut, Q, Nq, M, K, codes, offsets, B, total_tokens, scores, workspace, workspace_bytes, stream,
+                       variant);
+}
+
+size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B) {
+    (void)B;
+    if (Q <= 0 || Nq <= 0 || M != 16 || K != 256 || Nq % 8 != 0) return 0;  // general kernel: no scratch
+    return pq_smem_workspace_bytes(Q, Nq);
+}
+
+uint64_t tms_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char* tms_status_string(int status) {
+    switch (status) {
+        case TMS_OK: return "ok";
+        case TMS_ERR_INVALID_ARG: return "invalid argument";
+        case TMS_ERR_UNSUPPORTED: return "unsupported shape, dtype or device";
+        case TMS_ERR_ALIGNMENT: return "pointer or row pitch not 16-byte aligned";
+        case TMS_ERR_WORKSPACE: return "workspace missing or too small";
+        case TMS_ERR_CUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+int tms_version(void) { return 100; }
+
+}  // extern "C"

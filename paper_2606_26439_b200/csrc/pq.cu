@@ -1,0 +1,318 @@
+// pq.cu -- product-quantisation path: LUT build (Eq. 8), general fused lookup kernel, and the
+// shared-memory-resident LUT kernel (Eq. 9).
+//
+// The paper's phase 2 runs one program per (document, query token) with the table served from L2
+// (P:L268-270).  On B200 the lookups, not HBM, bound this path: Q*Nq*T*M 4-byte gathers against 2 GB of
+// codes.  The main kernel therefore keeps a 128 KB slice of the table -- 8 query
+// rows x M=16 x K=256 -- resident in shared memory, laid out so that every LDS.128 of a quarter-warp hits
+// eight different 16-byte bank groups whatever the codes are, and walks all slices over a document chunk
+// while the chunk's codes stay in L2, so codes come from HBM once.  No decompressed vector ever exists.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "tms_internal.h"
+
+namespace tms {
+namespace {
+
+__device__ __forceinline__ float to_f32(float v) { return v; }
+__device__ __forceinline__ float to_f32(__half v) { return __half2float(v); }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Eq. 8: lut[q,i,m,k] = sum_s queries[q,i,m*dsub+s] * C[m,k,s]   (fp32 FMA, s ascending)
+// grid (Q*Nq, M), one thread per centroid k.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+pq_build_lut_kernel(const T* __restrict__ queries, int d, const float* __restrict__ codebooks, int M, int K,
+                    float* __restrict__ lut) {
+    const int row = blockIdx.x, m = blockIdx.y, dsub = d / M;
+    const T* q = queries + (int64_t)row * d + m * dsub;
+    for (int k = threadIdx.x; k < K; k += blockDim.x) {
+        const float* c = codebooks + ((int64_t)m * K + k) * dsub;
+        float acc = 0.f;
+        for (int s = 0; s < dsub; ++s) acc = fmaf(to_f32(q[s]), c[s], acc);
+        lut[((int64_t)row * M + m) * K + k] = acc;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// General fused lookup kernel (TMS_VARIANT_SIMT): any M, any K <= 256, any Nq.  One CTA per document
+// (grid-stride), one thread per query row, table read through L1/L2 as in the paper.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int SIMT_THREADS = 256;
+constexpr int SIMT_TOK = 128;  // tokens staged per pass
+
+__global__ void __launch_bounds__(SIMT_THREADS)
+pq_simt_kernel(const float* __restrict__ lut, int Q, int Nq, int M, int K, const uint8_t* __restrict__ codes,
+               const int64_t* __restrict__ offsets, int64_t B, float* __restrict__ scores) {
+    extern __shared__ unsigned char smem_raw[];
+    const int R = Q * Nq;
+    float* rowmax = reinterpret_cast<float*>(smem_raw);                    // [R]
+    uint8_t* cs = smem_raw + sizeof(float) * (size_t)((R + 3) & ~3);       // [SIMT_TOK * M]
+    const int tid = threadIdx.x;
+    for (int64_t b = blockIdx.x; b < B; b += gridDim.x) {
+        const int64_t t0 = offsets[b], nd = offsets[b + 1] - t0;
+        for (int r = tid; r < R; r += SIMT_THREADS) rowmax[r] = -INFINITY;
+        for (int64_t j0 = 0; j0 < nd; j0 += SIMT_TOK) {
+            const int nt = (int)((nd - j0) < SIMT_TOK ? (nd - j0) : SIMT_TOK);
+            __syncthreads();
+            for (int e = tid; e < nt * M; e += SIMT_THREADS) cs[e] = codes[(t0 + j0) * M + e];
+            __syncthreads();
+            for (int r = tid; r < R; r += SIMT_THREADS) {
+                const float* lr = lut + (int64_t)r * M * K;
+                float mx = rowmax[r];
+                for (int j = 0; j < nt; ++j) {
+                    float s = 0.f;
+                    for (int m = 0; m < M; ++m) s += lr[m * K + cs[j * M + m]];  // Eq. 9, m ascending
+                    mx = fmaxf(mx, s);
+                }
+                rowmax[r] = mx;
+            }
+        }
+        __syncthreads();
+        for (int q = tid; q < Q; q += SIMT_THREADS) {
+            float s = 0.f;
+            for (int i = 0; i < Nq; ++i) s += rowmax[q * Nq + i];
+            scores[(int64_t)q * B + b] = s;
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Shared-memory-resident LUT kernel (TMS_VARIANT_PQ_SMEM): M = 16, K = 256, Nq % 8 == 0.
+//
+// Slice sl holds query rows 8*sl .. 8*sl+7.  Slice layout (floats), one 128-byte line per (m/4, k):
+//     line = (m >> 2) * 256 + k ;  within the line: [m & 3][row 0..7]
+// A warp handles 16 document tokens per step: lane = 8*s4 + 2*u + h  ->  token slot 4*s4 + u, rows 4h..4h+3.
+// At step (g, s) the lane looks up sub-quantiser m = 4g + ((s + u) & 3): the eight lanes of a quarter-warp
+// then read 16-byte pieces 2*((s+u)&3) + h of their (code-dependent) lines -- eight distinct bank groups,
+// conflict-free for any codes.  The per-lane order of the 16 additions is a fixed rotation of m.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int PQS_M = 16, PQS_K = 256, PQS_ROWS = 8;
+constexpr int PQS_SLICE_FLOATS = PQS_ROWS * PQS_M * PQS_K;  // 32768 floats = 128 KB
+constexpr int PQS_SLICE_BYTES = PQS_SLICE_FLOATS * 4;
+constexpr int PQS_WARPS = 16, PQS_THREADS = PQS_WARPS * 32;
+constexpr int PQS_MAX_SC_FLOATS = 20480;  // 80 KB of per-chunk score accumulators
+
+// lut [R, 16, 256] -> lutT [R/8 slices][4 g][256 k][4 sub][8 rows]
+__global__ void pq_relayout_kernel(const float* __restrict__ lut, float* __restrict__ lutT, int64_t total) {
+    const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= total) return;
+    const int row = (int)(o & 7), sub = (int)((o >> 3) & 3), k = (int)((o >> 5) & 255), g = (int)((o >> 13) & 3);
+    const int64_t sl = o >> 15;
+    lutT[o] = lut[((sl * 8 + row) * PQS_M + (4 * g + sub)) * PQS_K + k];
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
+__device__ __forceinline__ uint4 ldg_codes(const uint8_t* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+__global__ void __launch_bounds__(PQS_THREADS, 1)
+pq_smem_kernel(const float* __restrict__ lutT, int Q, int Nq, const uint8_t* __restrict__ codes,
+               const int64_t* __restrict__ offsets, int64_t B, int dpc /* docs per chunk */, int64_t nchunks,
+               float* __restrict__ scores) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* lut_s = reinterpret_cast<float*>(smem_raw);                          // 128 KB slice
+    float* sc = reinterpret_cast<float*>(smem_raw + PQS_SLICE_BYTES);           // [Q][dpc]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + PQS_SLICE_BYTES + sizeof(float) * PQS_MAX_SC_FLOATS);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int s4 = lane >> 3, u = (lane >> 1) & 3, h = lane & 1;
+    const int slot = s4 * 4 + u;
+    const int nslices = (Q * Nq) / PQS_ROWS;
+    const uint32_t bar_a = smem_u32(bar);
+    const uint32_t lut_a = smem_u32(lut_s);
+
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_a));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // per-lane constants: byte selector and 16-byte piece for each rotation step s
+    uint32_t sel[4], base[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+        const uint32_t sub = (uint32_t)((s + u) & 3);
+        sel[s] = 0x4440u | sub;  // PRMT: byte `sub` of the code word into bits 0..7, zeros above
+        base[s] = lut_a + sub * 32u + (uint32_t)h * 16u;
+    }
+    uint32_t phase = 0;
+    __syncthreads();
+
+    for (int64_t chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+        const int64_t d0 = chunk * dpc;
+        const int nd = (int)((B - d0) < dpc ? (B - d0) : dpc);
+        for (int sl = 0; sl < nslices; ++sl) {
+            __syncthreads();  // every warp is done reading the previous slice (and, at sl == 0, done with sc)
+            if (tid == 0) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a),
+                             "r"((uint32_t)PQS_SLICE_BYTES)
+                             : "memory");
+                const float* src = lutT + (int64_t)sl * PQS_SLICE_FLOATS;
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+                    asm volatile(
+                        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                            lut_a + p * (PQS_SLICE_BYTES / 4)),
+                        "l"(src + p * (PQS_SLICE_FLOATS / 4)), "r"((uint32_t)(PQS_SLICE_BYTES / 4)), "r"(bar_a)
+                        : "memory");
+            }
+            mbar_wait(bar_a, phase);
+            phase ^= 1;
+
+            const int q = (sl * PQS_ROWS) / Nq;
+            const bool first = (sl * PQS_ROWS) % Nq == 0;
+            for (int dd = warp; dd < nd; dd += PQS_WARPS) {
+                const int64_t t0 = offsets[d0 + dd];
+                const int n = (int)(offsets[d0 + dd + 1] - t0);
+                const uint8_t* cp = codes + (t0 + slot) * PQS_M;
+                float r0 = -INFINITY, r1 = -INFINITY, r2 = -INFINITY, r3 = -INFINITY;
+                uint4 c = make_uint4(0, 0, 0, 0);
+                if (slot < n) c = ldg_codes(cp);
+                for (int tb = 0; tb < n; tb += 16) {
+                    uint4 cn = make_uint4(0, 0, 0, 0);
+                    if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M);  // prefetch next step
+                    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+                    const uint32_t w[4] = {c.x, c.y, c.z, c.w};
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+#pragma unroll
+                        for (int s = 0; s < 4; ++s) {
+                            const uint32_t code = __byte_perm(w[g], 0u, sel[s]);
+                            const float4 v = lds128(base[s] + code * 128u + (uint32_t)g * (PQS_K * 128u));
+                            a0 += v.x; a1 += v.y; a2 += v.z; a3 += v.w;
+                        }
+                    }
+                    if (tb + slot < n) {
+                        r0 = fmaxf(r0, a0); r1 = fmaxf(r1, a1); r2 = fmaxf(r2, a2); r3 = fmaxf(r3, a3);
+                    }
+                    c = cn;
+                }
+                // max over the 16 token slots (lane bits 1..4), then sum of the 8 rows (4 here, 4 in lane ^ 1)
+#pragma unroll
+                for (int o = 2; o <= 16; o <<= 1) {
+                    r0 = fmaxf(r0, __shfl_xor_sync(0xffffffffu, r0, o));
+                    r1 = fmaxf(r1, __shfl_xor_sync(0xffffffffu, r1, o));
+                    r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+                    r3 = fmaxf(r3, __shfl_xor_sync(0xffffffffu, r3, o));
+                }
+                float part = (r0 + r1) + (r2 + r3);
+                part += __shfl_xor_sync(0xffffffffu, part, 1);
+                if (lane == 0) {
+                    float* dst = sc + q * dpc + dd;
+                    *dst = first ? part : (*dst + part);
+                }
+            }
+        }
+        __syncthreads();
+        for (int idx = tid; idx < Q * nd; idx += PQS_THREADS) {
+            const int q = idx / nd, dd = idx - q * nd;
+            scores[(int64_t)q * B + d0 + dd] = sc[q * dpc + dd];
+        }
+    }
+}
+
+}  // namespace
+
+int launch_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                        int K, float* lut, cudaStream_t stream) {
+    dim3 grid((unsigned)(Q * Nq), (unsigned)M);
+    switch (q_dtype) {
+        case TMS_DTYPE_F32:
+            pq_build_lut_kernel<float><<<grid, 256, 0, stream>>>(static_cast<const float*>(queries), d, codebooks,
+                                                                  M, K, lut);
+            break;
+        case TMS_DTYPE_F16:
+            pq_build_lut_kernel<__half><<<grid, 256, 0, stream>>>(static_cast<const __half*>(queries), d,
+                                                                   codebooks, M, K, lut);
+            break;
+        case TMS_DTYPE_BF16:
+            pq_build_lut_kernel<__nv_bfloat16><<<grid, 256, 0, stream>>>(
+                static_cast<const __nv_bfloat16*>(queries), d, codebooks, M, K, lut);
+            break;
+        default: return TMS_ERR_INVALID_ARG;
+    }
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
+}
+
+int launch_pq_simt(const PqArgs& a) {
+    const DeviceInfo* di = device_info();
+    if (!di) return TMS_ERR_CUDA;
+    if (a.B == 0) return TMS_OK;
+    const int R = a.Q * a.Nq;
+    const size_t smem = sizeof(float) * (size_t)((R + 3) & ~3) + (size_t)SIMT_TOK * a.M;
+    if (smem > 200 * 1024) return TMS_ERR_UNSUPPORTED;
+    if (smem > 40 * 1024 &&
+        cudaFuncSetAttribute(pq_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return TMS_ERR_CUDA;
+    const int64_t grid = a.B < (int64_t)di->num_sms * 8 ? a.B : (int64_t)di->num_sms * 8;
+    pq_simt_kernel<<<(unsigned)grid, SIMT_THREADS, smem, a.stream>>>(a.lut, a.Q, a.Nq, a.M, a.K, a.codes, a.offsets,
+                                                                     a.B, a.scores);
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
+}
+
+bool pq_smem_supports(const PqArgs& a) {
+    return a.M == PQS_M && a.K == PQS_K && a.Nq % PQS_ROWS == 0 && a.Q >= 1 && a.Q <= PQS_MAX_SC_FLOATS / 16;
+}
+
+size_t pq_smem_workspace_bytes(int Q, int Nq) { return sizeof(float) * (size_t)Q * Nq * PQS_M * PQS_K; }
+
+// workspace: the re-laid-out table lutT, same size as lut.
+int launch_pq_smem(const PqArgs& a, void* workspace) {
+    const DeviceInfo* di = device_info();
+    if (!di) return TMS_ERR_CUDA;
+    if (a.B == 0) return TMS_OK;
+    float* lutT = static_cast<float*>(workspace);
+    const int64_t total = (int64_t)a.Q * a.Nq * PQS_M * PQS_K;
+    pq_relayout_kernel<<<(unsigned)((total + 255) / 256), 256, 0, a.stream>>>(a.lut, lutT, total);
+    count_launch();
+    if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+
+    // docs per chunk: as large as the smem score accumulators allow (amortises the 128 KB slice reloads),
+    // but no larger than one CTA's share of a small batch
+    int dpc_max = PQS_MAX_SC_FLOATS / a.Q;
+    if (dpc_max > 256) dpc_max = 256;
+    int64_t dpc = (a.B + di->num_sms - 1) / di->num_sms;
+    if (dpc < 16) dpc = 16;
+    if (dpc > dpc_max) dpc = dpc_max;
+    const int64_t nchunks = (a.B + dpc - 1) / dpc;
+    const size_t smem = (size_t)PQS_SLICE_BYTES + sizeof(float) * PQS_MAX_SC_FLOATS + 16;
+    if (cudaFuncSetAttribute(pq_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return TMS_ERR_CUDA;
+    const int64_t grid = nchunks < di->num_sms ? nchunks : di->num_sms;
+    pq_smem_kernel<<<(unsigned)grid, PQS_THREADS, smem, a.stream>>>(lutT, a.Q, a.Nq, a.codes, a.offsets, a.B,
+                                                                    (int)dpc, nchunks, a.scores);
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
+}
+
+}  // namespace tms

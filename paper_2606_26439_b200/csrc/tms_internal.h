@@ -1,0 +1,60 @@
+// Internal declarations shared by the translation units of libtms.so (never installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/tms.h"
+
+namespace tms {
+
+inline size_t dtype_size(tms_dtype t) { return t == TMS_DTYPE_F32 ? 4 : 2; }
+
+// Every kernel launch in the library goes through this counter (tms_launch_count()).
+void count_launch(int n = 1);
+
+struct DeviceInfo {
+    int device = -1;
+    int cc_major = 0, cc_minor = 0;
+    int num_sms = 0;
+    int max_smem_optin = 0;
+};
+// Cached per device; returns nullptr when no CUDA device is usable.
+const DeviceInfo* device_info();
+
+// ---- dense -----------------------------------------------------------------------------------------------------
+struct DenseArgs {
+    const void* queries;
+    int Q, Nq, d;
+    const void* docs;
+    const int64_t* offsets;
+    int64_t B, T;
+    tms_dtype dtype;
+    float* scores;
+    cudaStream_t stream;
+};
+
+// CUDA-core tiled kernel: any dtype / d / Nq / Q (csrc/dense_simt.cu).
+int launch_dense_simt(const DenseArgs& a);
+// TMA + tcgen05 kernel (csrc/dense_tc.cu). supports() says whether the shape is covered.
+bool dense_tc_supports(const DenseArgs& a);
+int launch_dense_tc(const DenseArgs& a);
+
+// ---- PQ --------------------------------------------------------------------------------------------------------
+struct PqArgs {
+    const float* lut;
+    int Q, Nq, M, K;
+    const uint8_t* codes;
+    const int64_t* offsets;
+    int64_t B, T;
+    float* scores;
+    cudaStream_t stream;
+};
+int launch_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                        int K, float* lut, cudaStream_t stream);
+int launch_pq_simt(const PqArgs& a);
+bool pq_smem_supports(const PqArgs& a);
+size_t pq_smem_workspace_bytes(int Q, int Nq);
+int launch_pq_smem(const PqArgs& a, void* workspace);
+
+}  // namespace tms

@@ -1,0 +1,189 @@
+"""Thin ctypes binding over libtms.so: same names as include/tms.h, argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the hot path runs inside the library's
+CUDA kernels.  There is no fallback: if libtms.so is missing or a call fails, a RuntimeError is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtms.so")
+
+TMS_OK = 0
+TMS_DTYPE_F32, TMS_DTYPE_F16, TMS_DTYPE_BF16 = 0, 1, 2
+TMS_VARIANT_AUTO, TMS_VARIANT_SIMT, TMS_VARIANT_TCGEN05, TMS_VARIANT_PQ_SMEM = 0, 1, 2, 3
+VARIANTS = {"auto": 0, "simt": 1, "tcgen05": 2, "pq_smem": 3}
+
+_DTYPES = {torch.float32: TMS_DTYPE_F32, torch.float16: TMS_DTYPE_F16, torch.bfloat16: TMS_DTYPE_BF16}
+
+# every symbol include/tms.h declares: (restype, argtypes)
+_vp, _i, _i64, _sz, _u64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_size_t, ctypes.c_uint64
+SIGNATURES = {
+    "tms_maxsim": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
+    "tms_maxsim_variant": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp, _i]),
+    "tms_maxsim_workspace_bytes": (_sz, [_i, _i, _i, _i64, _i]),
+    "tms_pq_build_lut": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp]),
+    "tms_pq_maxsim": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
+    "tms_pq_maxsim_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
+    "tms_pq_workspace_bytes": (_sz, [_i, _i, _i, _i, _i64]),
+    "tms_maxsim_host": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
+    "tms_pq_maxsim_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
+    "tms_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i64]),
+    "tms_pq_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i, _i, _i64]),
+    "tms_launch_count": (_u64, []),
+    "tms_status_string": (ctypes.c_char_p, [_i]),
+    "tms_version": (_i, []),
+}
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Load libtms.so (built by `python -m paper_2606_26439_b200.build`); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_2606_26439_b200.build` "
+                               "(there is no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _check(status: int, what: str) -> None:
+    if status != TMS_OK:
+        raise RuntimeError(f"{what} failed: {load().tms_status_string(status).decode()} (status {status})")
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev(t: torch.Tensor, name: str) -> int:
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous CUDA tensor")
+    return t.data_ptr()
+
+
+def tms_launch_count() -> int:
+    return int(load().tms_launch_count())
+
+
+def tms_version() -> int:
+    return int(load().tms_version())
+
+
+def tms_maxsim_workspace_bytes(Q, Nq, d, B, dtype) -> int:
+    return int(load().tms_maxsim_workspace_bytes(Q, Nq, d, B, _DTYPES[dtype]))
+
+
+def tms_pq_workspace_bytes(Q, Nq, M, K, B) -> int:
+    return int(load().tms_pq_workspace_bytes(Q, Nq, M, K, B))
+
+
+def tms_maxsim(queries: torch.Tensor, docs: torch.Tensor, offsets: torch.Tensor, scores: torch.Tensor | None = None,
+               stream=None, variant: str = "auto") -> torch.Tensor:
+    """scores[q,b] = sum_i max_{t in doc b} <queries[q,i], docs[t]>  (include/tms.h: tms_maxsim)."""
+    Q, Nq, d = queries.shape
+    T = docs.shape[0]
+    B = offsets.numel() - 1
+    if docs.dim() != 2 or docs.shape[1] != d or docs.dtype != queries.dtype or offsets.dtype != torch.int64:
+        raise ValueError("docs must be [T,d] in the queries' dtype and offsets int64 [B+1]")
+    if scores is None:
+        scores = torch.empty((Q, B), dtype=torch.float32, device=queries.device)
+    elif scores.shape != (Q, B) or scores.dtype != torch.float32:
+        raise ValueError("scores must be fp32 [Q,B]")
+    lib = load()
+    st = lib.tms_maxsim_variant(_dev(queries, "queries"), Q, Nq, d, _dev(docs, "docs") if T else None,
+                                _dev(offsets, "offsets"), B, T, _DTYPES[queries.dtype],
+                                _dev(scores, "scores") if B else None, None, 0, _stream(stream), VARIANTS[variant])
+    _check(st, "tms_maxsim")
+    return scores
+
+
+def tms_pq_build_lut(queries: torch.Tensor, codebooks: torch.Tensor, lut: torch.Tensor | None = None,
+                     stream=None) -> torch.Tensor:
+    """lut[q,i,m,k] = <queries[q,i,m-th slice], codebooks[m,k]>  (Eq. 8)."""
+    Q, Nq, d = queries.shape
+    M, K, dsub = codebooks.shape
+    if codebooks.dtype != torch.float32 or M * dsub != d:
+        raise ValueError("codebooks must be fp32 [M,K,d/M]")
+    if lut is None:
+        lut = torch.empty((Q, Nq, M, K), dtype=torch.float32, device=queries.device)
+    st = load().tms_pq_build_lut(_dev(queries, "queries"), Q, Nq, d, _DTYPES[queries.dtype],
+                                 _dev(codebooks, "codebooks"), M, K, _dev(lut, "lut"), _stream(stream))
+    _check(st, "tms_pq_build_lut")
+    return lut
+
+
+def tms_pq_maxsim(lut: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor, scores: torch.Tensor | None = None,
+                  workspace: torch.Tensor | None = None, stream=None, variant: str = "auto") -> torch.Tensor:
+    """scores[q,b] = sum_i max_{t in doc b} sum_m lut[q,i,m,codes[t,m]]  (Eq. 9)."""
+    Q, Nq, M, K = lut.shape
+    T = codes.shape[0]
+    B = offsets.numel() - 1
+    if codes.dtype != torch.uint8 or codes.dim() != 2 or codes.shape[1] != M or lut.dtype != torch.float32:
+        raise ValueError("codes must be uint8 [T,M] and lut fp32 [Q,Nq,M,K]")
+    if scores is None:
+        scores = torch.empty((Q, B), dtype=torch.float32, device=lut.device)
+    lib = load()
+    need = int(lib.tms_pq_workspace_bytes(Q, Nq, M, K, B))
+    if workspace is None and need:
+        workspace = torch.empty(need, dtype=torch.uint8, device=lut.device)
+    ws_ptr = _dev(workspace, "workspace") if workspace is not None else None
+    ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    st = lib.tms_pq_maxsim_variant(_dev(lut, "lut"), Q, Nq, M, K, _dev(codes, "codes") if T else None,
+                                   _dev(offsets, "offsets"), B, T, _dev(scores, "scores") if B else None, ws_ptr,
+                                   ws_len, _stream(stream), VARIANTS[variant])
+    _check(st, "tms_pq_maxsim")
+    return scores
+
+
+def _host(t: torch.Tensor, name: str) -> int:
+    if t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous host tensor")
+    return t.data_ptr()
+
+
+def tms_maxsim_host_workspace_min_bytes(Q, Nq, d, dtype, max_doc_tokens) -> int:
+    return int(load().tms_maxsim_host_workspace_min_bytes(Q, Nq, d, _DTYPES[dtype], max_doc_tokens))
+
+
+def tms_pq_maxsim_host_workspace_min_bytes(Q, Nq, d, q_dtype, M, K, max_doc_tokens) -> int:
+    return int(load().tms_pq_maxsim_host_workspace_min_bytes(Q, Nq, d, _DTYPES[q_dtype], M, K, max_doc_tokens))
+
+
+def tms_maxsim_host(queries: torch.Tensor, docs: torch.Tensor, offsets: torch.Tensor, scores: torch.Tensor,
+                    dev_workspace: torch.Tensor, stream=None) -> torch.Tensor:
+    """Same result with HOST tensors (pinned recommended); the store is streamed through dev_workspace."""
+    Q, Nq, d = queries.shape
+    T, B = docs.shape[0], offsets.numel() - 1
+    st = load().tms_maxsim_host(_host(queries, "queries"), Q, Nq, d, _host(docs, "docs"), _host(offsets, "offsets"),
+                                B, T, _DTYPES[queries.dtype], _host(scores, "scores"),
+                                _dev(dev_workspace, "dev_workspace"),
+                                dev_workspace.numel() * dev_workspace.element_size(), _stream(stream))
+    _check(st, "tms_maxsim_host")
+    return scores
+
+
+def tms_pq_maxsim_host(queries: torch.Tensor, codebooks: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor,
+                       scores: torch.Tensor, dev_workspace: torch.Tensor, stream=None) -> torch.Tensor:
+    Q, Nq, d = queries.shape
+    M, K, _ = codebooks.shape
+    T, B = codes.shape[0], offsets.numel() - 1
+    st = load().tms_pq_maxsim_host(_host(queries, "queries"), Q, Nq, d, _DTYPES[queries.dtype],
+                                   _host(codebooks, "codebooks"), M, K, _host(codes, "codes"),
+                                   _host(offsets, "offsets"), B, T, _host(scores, "scores"),
+                                   _dev(dev_workspace, "dev_workspace"),
+                                   dev_workspace.numel() * dev_workspace.element_size(), _stream(stream))
+    _check(st, "tms_pq_maxsim_host")
+    return scores

@@ -1,0 +1,101 @@
+"""GPU parity for the PQ path: tms_pq_build_lut (Eq. 8) and tms_pq_maxsim (Eq. 9) against the oracle's
+explicit decompress-then-score.  Queries are bf16, so the tolerance is 2e-3*Nq."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_26439_b200 import synth, tms
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def pq_case(Q, Nq, M, K, dsub, off, seed, q_dtype=torch.bfloat16):
+    d = M * dsub
+    q = synth.unit_tokens(Q * Nq, d, q_dtype, seed=seed).view(Q, Nq, d)
+    C = synth.pq_codebooks(M, K, dsub, seed=seed + 1)
+    codes = synth.pq_codes(int(off[-1]), M, seed=seed + 2, K=K)
+    return q, C, codes
+
+
+def run_pq(q, C, codes, off, variant="auto"):
+    lut = tms.tms_pq_build_lut(q.to(DEV), C.to(DEV))
+    out = tms.tms_pq_maxsim(lut, codes.to(DEV), torch.from_numpy(off).to(DEV), variant=variant)
+    torch.cuda.synchronize()
+    return lut.cpu().numpy(), out.cpu().numpy().astype(np.float64)
+
+
+def assert_close(got, ref, atol):
+    inf = np.isneginf(ref)
+    assert np.array_equal(np.isneginf(got), inf)
+    err = np.abs(got[~inf] - ref[~inf])
+    assert err.size == 0 or err.max() <= atol, f"max |dscore| = {err.max():.3e} > {atol:.3e}"
+
+
+@pytest.mark.parametrize("q_dtype", [torch.bfloat16, torch.float16, torch.float32])
+def test_lut_matches_eq8_in_fp64(q_dtype):
+    off = synth.uniform_offsets(1, 1)
+    q, C, codes = pq_case(8, 32, 16, 256, 8, off, seed=1, q_dtype=q_dtype)
+    lut, _ = run_pq(q, C, codes, off)
+    ref = np.einsum("qims,mks->qimk", q.to(torch.float64).numpy().reshape(8, 32, 16, 8), C.to(torch.float64).numpy())
+    assert np.abs(lut - ref).max() < 2e-6  # fp32 FMA chain of 8 terms, |terms| < 1
+
+
+@pytest.mark.parametrize("variant", ["simt", "pq_smem"])
+def test_config4_shape_small(variant):
+    off = synth.uniform_offsets(3000, 128)
+    q, C, codes = pq_case(8, 32, 16, 256, 8, off, seed=3)
+    _, got = run_pq(q, C, codes, off, variant)
+    assert_close(got, oracle.pq_maxsim(q, C, codes, off), 2e-3 * 32)
+    assert 28.0 < got.mean() < 31.0
+
+
+@pytest.mark.parametrize("variant", ["simt", "pq_smem"])
+def test_ragged_documents(variant):
+    lens = np.concatenate([[5, 128, 1, 0, 300, 16, 17, 15, 0, 0, 33, 1000],
+                           synth.lognormal_lengths(2000, seed=2, median=40, lo=0, hi=200)])
+    off = synth.offsets_from_lengths(lens)
+    q, C, codes = pq_case(3, 32, 16, 256, 8, off, seed=5)
+    _, got = run_pq(q, C, codes, off, variant)
+    assert_close(got, oracle.pq_maxsim(q, C, codes, off), 2e-3 * 32)
+
+
+@pytest.mark.parametrize("Q,Nq,M,K,dsub", [(2, 12, 8, 64, 4), (1, 32, 32, 256, 4), (5, 7, 16, 256, 8)])
+def test_general_shapes_take_the_general_kernel(Q, Nq, M, K, dsub):
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(300, seed=4, median=30, lo=0, hi=100))
+    q, C, codes = pq_case(Q, Nq, M, K, dsub, off, seed=7)
+    _, got = run_pq(q, C, codes, off, "auto")
+    assert_close(got, oracle.pq_maxsim(q, C, codes, off), 2e-3 * Nq)
+
+
+def test_smem_and_general_kernels_agree_and_are_reproducible():
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(5000, seed=9))
+    q, C, codes = pq_case(8, 32, 16, 256, 8, off, seed=11)
+    _, a = run_pq(q, C, codes, off, "pq_smem")
+    _, a2 = run_pq(q, C, codes, off, "pq_smem")
+    _, b = run_pq(q, C, codes, off, "simt")
+    assert np.array_equal(a, a2)
+    assert np.abs(a - b).max() < 1e-4  # same fp32 terms, different summation order over m
+
+
+def test_p13_lossless_codes_reproduce_the_dense_path():
+    """Documents whose sub-vectors ARE centroids: the PQ score equals the dense fp32 score of those vectors."""
+    M, K, dsub, B, Nd = 16, 256, 8, 400, 64
+    off = synth.uniform_offsets(B, Nd)
+    q, C, codes = pq_case(4, 32, M, K, dsub, off, seed=13, q_dtype=torch.float32)
+    dhat = torch.stack([C[m, codes[:, m].long()] for m in range(M)], dim=1).reshape(B * Nd, M * dsub)
+    _, pq = run_pq(q, C, codes, off, "pq_smem")
+    dense = tms.tms_maxsim(q.to(DEV), dhat.to(DEV), torch.from_numpy(off).to(DEV)).cpu().numpy()
+    assert np.abs(pq - dense).max() < 1e-5 * 32 * 4  # |dhat| ~ 4: scale the fp32 tolerance by the score magnitude
+
+
+def test_host_entry_point():
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(6000, seed=15))
+    q, C, codes = pq_case(8, 32, 16, 256, 8, off, seed=17)
+    _, ref = run_pq(q, C, codes, off)
+    scores = torch.empty((8, 6000), dtype=torch.float32).pin_memory()
+    need = tms.tms_pq_maxsim_host_workspace_min_bytes(8, 32, 128, torch.bfloat16, 16, 256, 180)
+    ws = torch.empty(need + (2 << 20), dtype=torch.uint8, device=DEV)  # ~1 MB per chunk buffer: several chunks
+    tms.tms_pq_maxsim_host(q, C, codes.pin_memory(), torch.from_numpy(off), scores, ws)
+    assert np.array_equal(scores.numpy().astype(np.float64), ref)
