@@ -165,6 +165,34 @@ struct SegInfo {
     uint32_t doc[BN];     // k-th set bit  ->  document index relative to the CTA's first document
 };
 
+// Eight accumulator columns in which at least one document ends (bit j of b8: column j is a document's last
+// token).  Out of line on purpose: boundary chunks are the minority, and keeping one copy of this code keeps the
+// epilogue's hot loop inside the instruction cache.  Running max per row; at a boundary the Nq maxima of each query
+// are summed across lanes in a fixed xor-shuffle order and lane i == 0 stores the score (Eq. 1).
+// flags: bits 0-7 Nq_pad (a power of two <= 32), bit 8 row holds a real query token, bit 9 row writes the score.
+__device__ __noinline__ uint2 epi_boundary_chunk(float x0, float x1, float x2, float x3, float x4, float x5, float x6,
+                                                 float x7, uint32_t b8, float m, uint32_t k, uint32_t flags,
+                                                 const uint32_t* doc, float* out) {
+    const float x[8] = {x0, x1, x2, x3, x4, x5, x6, x7};
+    const uint32_t nqp = flags & 0xffu;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        m = fmaxf(m, x[j]);
+        if (b8 & (1u << j)) {
+            float v = (flags & 0x100u) ? m : 0.f;
+            if (nqp > 16) v += __shfl_xor_sync(0xffffffffu, v, 16);
+            if (nqp > 8) v += __shfl_xor_sync(0xffffffffu, v, 8);
+            if (nqp > 4) v += __shfl_xor_sync(0xffffffffu, v, 4);
+            if (nqp > 2) v += __shfl_xor_sync(0xffffffffu, v, 2);
+            if (nqp > 1) v += __shfl_xor_sync(0xffffffffu, v, 1);
+            if (flags & 0x200u) out[doc[k]] = v;
+            ++k;
+            m = -INFINITY;
+        }
+    }
+    return make_uint2(__float_as_uint(m), k);
+}
+
 template <bool TF32>
 __global__ void __launch_bounds__(384, 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_constant__ CUtensorMap map_q,
@@ -250,16 +278,16 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
                     tma_load_2d(smem_u32(a_ptr + (size_t)(mb * p.NKB + kb) * A_BLOCK_BYTES + r * KB_BYTES), &map_q,
                                 smem_u32(qfull), kb * p.kb_elems, q * p.Nq, pol_q);
             }
-            uint32_t it = 0;
+            uint32_t s = 0, ph = 0;  // ring slot and its phase bit
             for (int64_t t = 0; t < ntiles; ++t) {
                 const int tok = (int)(t_lo + t * BN);
-                for (int ch = 0; ch < nchunks; ++ch, ++it) {
-                    const uint32_t s = it % p.NS, ph = (it / p.NS) & 1;
+                for (int ch = 0; ch < nchunks; ++ch) {
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
                     mbar_expect_tx(smem_u32(full + s), stage_bytes);
                     for (int k = 0; k < p.KBS; ++k)
                         tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
                                     smem_u32(full + s), (ch * p.KBS + k) * p.kb_elems, tok, pol_docs);
+                    if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
                 }
             }
         }
@@ -270,14 +298,12 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
             mbar_wait(smem_u32(qfull), 0);
             tc_fence_after();
             const uint32_t a_base = smem_u32(a_ptr);
-            uint32_t it = 0;
+            uint32_t s = 0, ph = 0, ts = 0, tph = 0;
             for (int64_t t = 0; t < ntiles; ++t) {
-                const uint32_t ts = (uint32_t)(t % p.NT), tph = (uint32_t)((t / p.NT) & 1);
                 mbar_wait(smem_u32(tempty + ts), tph ^ 1);  // epilogue has drained this accumulator stage
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + ts * (uint32_t)(p.MB * BN);
-                for (int ch = 0; ch < nchunks; ++ch, ++it) {
-                    const uint32_t s = it % p.NS, ph = (it / p.NS) & 1;
+                for (int ch = 0; ch < nchunks; ++ch) {
                     mbar_wait(smem_u32(full + s), ph);
                     tc_fence_after();
                     const uint32_t b_base = smem_u32(st_ptr + (size_t)s * stage_bytes);
@@ -294,27 +320,39 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
                         }
                     }
                     tc_commit(smem_u32(empty + s));  // frees the smem stage once these MMAs have read it
+                    if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
                 }
                 tc_commit(smem_u32(tfull + ts));     // accumulator stage complete -> epilogue
+                if (++ts == (uint32_t)p.NT) { ts = 0; tph ^= 1; }
             }
         }
         __syncwarp();
     } else if (warp == 2) {
         // ===== document segmenter =====
-        int64_t b = b_lo;
+        // Lane l holds the end offset of document wb + l (a 32-document window in registers); the next window is
+        // loaded one window ahead, so no tile waits on a global load.  A document's start is its predecessor's end.
         const uint32_t lt_mask = (1u << lane) - 1u;
         const float ninf = -INFINITY;
+        const int64_t never = INT64_MAX;
+        auto load_ends = [&](int64_t base) -> int64_t {
+            const int64_t idx = base + lane;
+            return idx < b_hi ? p.offsets[idx + 1] : never;
+        };
+        int64_t wb = b_lo;
+        int64_t e_cur = load_ends(wb), e_nxt = load_ends(wb + 32);
+        int64_t s_first = t_lo;  // start of document wb
+        int consumed = 0;        // documents of the current window already assigned to a tile
         for (int64_t t = 0; t < ntiles; ++t) {
             const uint32_t g = (uint32_t)(t % NSEG), gph = (uint32_t)((t / NSEG) & 1);
             const int64_t tile_start = t_lo + t * BN, tile_end = tile_start + BN;
             mbar_wait(smem_u32(sempty + g), gph ^ 1);
             uint32_t m0 = 0, m1 = 0, m2 = 0, m3 = 0, nseg = 0;
             while (true) {
-                const int64_t idx = b + lane;
-                const bool valid = idx < b_hi;
-                const int64_t e = valid ? p.offsets[idx + 1] : 0;
-                const int64_t s = valid ? p.offsets[idx] : 0;
-                const bool in_tile = valid && e <= tile_end;  // ends are monotone: a prefix of the lanes
+                const int64_t idx = wb + lane;
+                const int64_t e = e_cur;
+                const int64_t e_prev = __shfl_up_sync(0xffffffffu, e_cur, 1);
+                const int64_t s = lane == 0 ? s_first : e_prev;
+                const bool in_tile = lane >= consumed && e <= tile_end;  // ends are monotone: a run of lanes
                 const unsigned ball = __ballot_sync(0xffffffffu, in_tile);
                 const bool nonempty = in_tile && e > s;
                 const unsigned nb = __ballot_sync(0xffffffffu, nonempty);
@@ -328,19 +366,25 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
                 } else if (in_tile) {
                     for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;  // empty document (A2)
                 }
-                m0 |= __reduce_or_sync(0xffffffffu, w0); m1 |= __reduce_or_sync(0xffffffffu, w1);
-                m2 |= __reduce_or_sync(0xffffffffu, w2); m3 |= __reduce_or_sync(0xffffffffu, w3);
+                if (nb) {
+                    m0 |= __reduce_or_sync(0xffffffffu, w0); m1 |= __reduce_or_sync(0xffffffffu, w1);
+                    m2 |= __reduce_or_sync(0xffffffffu, w2); m3 |= __reduce_or_sync(0xffffffffu, w3);
+                }
                 nseg += __popc(nb);
-                const int cnt = __popc(ball);
-                b += cnt;
-                if (cnt < 32) break;
+                consumed += __popc(ball);
+                if (consumed < 32) break;
+                s_first = __shfl_sync(0xffffffffu, e_cur, 31);  // window exhausted: slide to the prefetched one
+                wb += 32;
+                e_cur = e_nxt;
+                e_nxt = load_ends(wb + 32);
+                consumed = 0;
             }
             if (lane == 0) { seg[g].mask[0] = m0; seg[g].mask[1] = m1; seg[g].mask[2] = m2; seg[g].mask[3] = m3; }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sfull + g));
         }
         // documents after the last token of the range can only be empty
-        for (int64_t idx = b + lane; idx < b_hi; idx += 32)
+        for (int64_t idx = wb + consumed + lane; idx < b_hi; idx += 32)
             for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
     } else if (warp >= 4) {
         // ===== epilogue: running rowmax, segmented by document; max -> sum =====
@@ -350,60 +394,61 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
         const bool row_valid = (q < p.Q) && (i < p.Nq);
         const bool writer = row_valid && (i == 0);
         float* out = p.scores + (int64_t)(q < p.Q ? q : 0) * p.B + b_lo;
-        const int nqp = p.Nq_pad;
+        const uint32_t flags = (uint32_t)p.Nq_pad | (row_valid ? 0x100u : 0u) | (writer ? 0x200u : 0u);
         float m = -INFINITY;  // Alg. 3 line 4
 
-        auto flush = [&](uint32_t g, uint32_t& k) {
-            float v = row_valid ? m : 0.f;
-            if (nqp > 16) v += __shfl_xor_sync(0xffffffffu, v, 16);
-            if (nqp > 8) v += __shfl_xor_sync(0xffffffffu, v, 8);
-            if (nqp > 4) v += __shfl_xor_sync(0xffffffffu, v, 4);
-            if (nqp > 2) v += __shfl_xor_sync(0xffffffffu, v, 2);
-            if (nqp > 1) v += __shfl_xor_sync(0xffffffffu, v, 1);
-            if (writer) out[seg[g].doc[k]] = v;
-            ++k;
-            m = -INFINITY;
-        };
-
+        const uint32_t nt = (uint32_t)p.NT, tstride = (uint32_t)(p.MB * BN);
+        const uint32_t taddr0 = tmem_base + ((uint32_t)(quad * 32) << 16) + mb * BN;
+        uint32_t ts = 0, tph = 0, g = 0, gph = 0;
         for (int64_t t = 0; t < ntiles; ++t) {
-            const uint32_t ts = (uint32_t)(t % p.NT), tph = (uint32_t)((t / p.NT) & 1);
-            const uint32_t g = (uint32_t)(t % NSEG), gph = (uint32_t)((t / NSEG) & 1);
             mbar_wait(smem_u32(tfull + ts), tph);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + ts * (uint32_t)(p.MB * BN) + mb * BN;
+            const uint32_t taddr = taddr0 + ts * tstride;
             float v[BN];
             tmem_ld32(taddr + 0, v + 0);
             tmem_ld32(taddr + 32, v + 32);
             tmem_ld32(taddr + 64, v + 64);
             tmem_ld32(taddr + 96, v + 96);
+            mbar_wait(smem_u32(sfull + g), gph);
+            const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
             tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(tempty + ts));  // accumulator stage is free again
-            mbar_wait(smem_u32(sfull + g), gph);
             uint32_t k = 0;
+            const uint32_t mw[4] = {mask.x, mask.y, mask.z, mask.w};
 #pragma unroll
             for (int c4 = 0; c4 < 4; ++c4) {
-                const uint32_t bits = seg[g].mask[c4];
+                const uint32_t bits = mw[c4];
+                if (bits == 0) {  // no document ends inside these 32 columns: a max tree, 3 inputs per instruction
+                    const float* x = v + c4 * 32;
+                    float a[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) a[j] = fmaxf(fmaxf(x[4 * j], x[4 * j + 1]), fmaxf(x[4 * j + 2], x[4 * j + 3]));
+                    const float b0 = fmaxf(fmaxf(a[0], a[1]), a[2]), b1 = fmaxf(fmaxf(a[3], a[4]), a[5]);
+                    m = fmaxf(fmaxf(m, b0), fmaxf(fmaxf(b1, a[6]), a[7]));
+                    continue;
+                }
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
                     const uint32_t b8 = (bits >> (8 * ch)) & 0xffu;
                     const float* x = v + c4 * 32 + ch * 8;
-                    if (b8 == 0) {
+                    if (b8 == 0) {  // no document ends inside these 8 columns
                         const float m01 = fmaxf(fmaxf(x[0], x[1]), x[2]);
                         const float m23 = fmaxf(fmaxf(x[3], x[4]), x[5]);
                         m = fmaxf(fmaxf(m, m01), fmaxf(fmaxf(m23, x[6]), x[7]));
                     } else {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            m = fmaxf(m, x[j]);
-                            if (b8 & (1u << j)) flush(g, k);
-                        }
+                        const uint2 r = epi_boundary_chunk(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], b8, m, k, flags,
+                                                           seg[g].doc, out);
+                        m = __uint_as_float(r.x);
+                        k = r.y;
                     }
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
+            if (++ts == nt) { ts = 0; tph ^= 1; }
+            if (++g == NSEG) { g = 0; gph ^= 1; }
         }
     }
 
