@@ -20,6 +20,7 @@
 // segmenter (turns `offsets` into per-tile boundary masks, writes -inf for empty documents), warp 3 idle,
 // warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of M-block (w-4)/4).
 #include <cuda.h>
+#include <cstdlib>
 #include <cuda_runtime.h>
 
 #include "tms_internal.h"
@@ -48,6 +49,7 @@ struct Params {
     int NT;        // TMEM accumulator stages = 512 / (MB*128)
     uint32_t idesc;
     int kb_elems;  // elements per dimension block (64 or 32)
+    int debug;     // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs
 };
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------
@@ -165,44 +167,78 @@ struct SegInfo {
     uint32_t doc[BN];     // k-th set bit  ->  document index relative to the CTA's first document
 };
 
-// Eight accumulator columns in which at least one document ends (bit j of b8: column j is a document's last
-// token).  Out of line on purpose: boundary chunks are the minority, and keeping one copy of this code keeps the
-// epilogue's hot loop inside the instruction cache.  Running max per row; at a boundary the Nq maxima of each query
-// are summed across lanes in a fixed xor-shuffle order and lane i == 0 stores the score (Eq. 1).
+// ---- epilogue helpers ------------------------------------------------------------------------------------------
 // flags: bits 0-7 Nq_pad (a power of two <= 32), bit 8 row holds a real query token, bit 9 row writes the score.
-__device__ __noinline__ uint2 epi_boundary_chunk(float x0, float x1, float x2, float x3, float x4, float x5, float x6,
-                                                 float x7, uint32_t b8, float m, uint32_t k, uint32_t flags,
-                                                 const uint32_t* doc, float* out) {
-    const float x[8] = {x0, x1, x2, x3, x4, x5, x6, x7};
+
+// max -> sum (Eq. 1): the Nq running maxima of one query sit in Nq adjacent lanes; they are summed in a fixed
+// xor-shuffle order and the lane of query token 0 stores the score of the k-th document that ends in this tile.
+__device__ __forceinline__ void flush_inline(float m, uint32_t k, uint32_t flags, const uint32_t* doc, float* out) {
     const uint32_t nqp = flags & 0xffu;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        m = fmaxf(m, x[j]);
-        if (b8 & (1u << j)) {
-            float v = (flags & 0x100u) ? m : 0.f;
-            if (nqp > 16) v += __shfl_xor_sync(0xffffffffu, v, 16);
-            if (nqp > 8) v += __shfl_xor_sync(0xffffffffu, v, 8);
-            if (nqp > 4) v += __shfl_xor_sync(0xffffffffu, v, 4);
-            if (nqp > 2) v += __shfl_xor_sync(0xffffffffu, v, 2);
-            if (nqp > 1) v += __shfl_xor_sync(0xffffffffu, v, 1);
-            if (flags & 0x200u) out[doc[k]] = v;
-            ++k;
-            m = -INFINITY;
-        }
-    }
-    return make_uint2(__float_as_uint(m), k);
+    float v = (flags & 0x100u) ? m : 0.f;
+    if (nqp > 16) v += __shfl_xor_sync(0xffffffffu, v, 16);
+    if (nqp > 8) v += __shfl_xor_sync(0xffffffffu, v, 8);
+    if (nqp > 4) v += __shfl_xor_sync(0xffffffffu, v, 4);
+    if (nqp > 2) v += __shfl_xor_sync(0xffffffffu, v, 2);
+    if (nqp > 1) v += __shfl_xor_sync(0xffffffffu, v, 1);
+    if (flags & 0x200u) out[doc[k]] = v;
+}
+__device__ __noinline__ void epi_flush(float m, uint32_t k, uint32_t flags, const uint32_t* doc, float* out) {
+    flush_inline(m, k, flags, doc, out);
 }
 
-template <bool TF32>
-__global__ void __launch_bounds__(384, 1)
+// max of 32 accumulator columns and the running max, three inputs per FMNMX3
+__device__ __forceinline__ float max_tree32(float m, const float* x) {
+    float a[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = fmaxf(fmaxf(x[4 * j], x[4 * j + 1]), fmaxf(x[4 * j + 2], x[4 * j + 3]));
+    const float b0 = fmaxf(fmaxf(a[0], a[1]), a[2]), b1 = fmaxf(fmaxf(a[3], a[4]), a[5]);
+    return fmaxf(fmaxf(m, b0), fmaxf(fmaxf(b1, a[6]), a[7]));
+}
+
+// 32 accumulator columns in which at least one document ends (bit c of `bits`: column c is a document's last token).
+// Out of line and re-reading its columns from TMEM on purpose: boundary words are the minority, and one compact copy
+// of this code keeps the epilogue's hot loop inside the instruction cache.  One iteration per document end: the
+// segment's columns are selected by predicate, folded into the running max, and the document is flushed.
+__device__ __noinline__ uint2 epi_boundary_word(uint32_t taddr, uint32_t bits, float m, uint32_t k, uint32_t flags,
+                                                const uint32_t* doc, float* out) {
+    float x[32];
+    tmem_ld32(taddr, x);
+    tmem_ld_wait();
+    uint32_t done = 0;  // columns that belong to documents already flushed
+    while (bits) {
+        const uint32_t low = bits & (0u - bits);
+        const uint32_t seg = ((low << 1) - 1u) & ~done;
+        float a0 = m, a1 = -INFINITY;
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) {
+            a0 = fmaxf(a0, (seg >> c) & 1u ? x[c] : -INFINITY);
+            a1 = fmaxf(a1, (seg >> (c + 1)) & 1u ? x[c + 1] : -INFINITY);
+        }
+        flush_inline(fmaxf(a0, a1), k, flags, doc, out);
+        ++k;
+        m = -INFINITY;
+        done |= seg;
+        bits ^= low;
+    }
+    float a0 = m, a1 = -INFINITY;
+#pragma unroll
+    for (int c = 0; c < 32; c += 2) {
+        a0 = fmaxf(a0, (done >> c) & 1u ? -INFINITY : x[c]);
+        a1 = fmaxf(a1, (done >> (c + 1)) & 1u ? -INFINITY : x[c + 1]);
+    }
+    return make_uint2(__float_as_uint(fmaxf(a0, a1)), k);
+}
+
+template <bool TF32, int MB, int KBS>
+__global__ void __launch_bounds__(128 + 128 * MB, 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_constant__ CUtensorMap map_q,
                 const Params p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     // layout: [A: MB*NKB*16 KB] [stages: NS * KBS*16 KB] [SegInfo x NSEG] [barriers] [misc]
-    const uint32_t a_bytes = (uint32_t)p.MB * p.NKB * A_BLOCK_BYTES;
-    const uint32_t stage_bytes = (uint32_t)p.KBS * KB_TILE_BYTES;
+    const uint32_t a_bytes = (uint32_t)MB * p.NKB * A_BLOCK_BYTES;
+    const uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
     uint8_t* a_ptr = smem;
     uint8_t* st_ptr = smem + a_bytes;
     SegInfo* seg = reinterpret_cast<SegInfo*>(st_ptr + (size_t)p.NS * stage_bytes);
@@ -219,7 +255,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
     int64_t* range = reinterpret_cast<int64_t*>(qfull + 2);  // b_lo, b_hi, t_lo, t_hi
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_epi_warps = 4 * p.MB;
+    const int n_epi_warps = 4 * MB;
 
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0) {
@@ -262,7 +298,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
     const uint32_t tmem_base = *tmem_slot;
     const int64_t b_lo = range[0], b_hi = range[1], t_lo = range[2], t_hi = range[3];
     const int64_t ntiles = (t_hi - t_lo + BN - 1) / BN;
-    const int nchunks = p.NKB / p.KBS;  // pipeline stages consumed per tile
+    const int nchunks = p.NKB / KBS;  // pipeline stages consumed per tile
 
     if (warp == 0) {
         // ===== TMA producer =====
@@ -284,9 +320,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
                 for (int ch = 0; ch < nchunks; ++ch) {
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
                     mbar_expect_tx(smem_u32(full + s), stage_bytes);
-                    for (int k = 0; k < p.KBS; ++k)
+                    for (int k = 0; k < KBS; ++k)
                         tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
-                                    smem_u32(full + s), (ch * p.KBS + k) * p.kb_elems, tok, pol_docs);
+                                    smem_u32(full + s), (ch * KBS + k) * p.kb_elems, tok, pol_docs);
                     if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
                 }
             }
@@ -294,31 +330,48 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
         __syncwarp();
     } else if (warp == 1) {
         // ===== MMA issuer =====
+        // One thread issues every tcgen05.mma of the CTA, so its instruction stream must stay short: the loops
+        // over K steps and query blocks are compile-time, and a descriptor is the previous one plus a constant.
         if (lane == 0) {
             mbar_wait(smem_u32(qfull), 0);
             tc_fence_after();
-            const uint32_t a_base = smem_u32(a_ptr);
+            constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);  // SBO 1024 B, version 1, SWIZZLE_128B
+            constexpr uint32_t DESC_LO = 1u << 16;                                // LBO field (unused for this layout)
+            const uint32_t a_lo0 = ((smem_u32(a_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
+            const uint32_t a_mb_step = (uint32_t)p.NKB * (A_BLOCK_BYTES >> 4);    // next 128-row query block
+            const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
+            const uint32_t stage_step = stage_bytes >> 4;
+            const uint32_t idesc = p.idesc;
+            const bool skip = (p.debug & 2) != 0;
             uint32_t s = 0, ph = 0, ts = 0, tph = 0;
             for (int64_t t = 0; t < ntiles; ++t) {
                 mbar_wait(smem_u32(tempty + ts), tph ^ 1);  // epilogue has drained this accumulator stage
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + ts * (uint32_t)(p.MB * BN);
+                const uint32_t d_tmem = tmem_base + ts * (uint32_t)(MB * BN);
+                uint32_t a_lo = a_lo0;
                 for (int ch = 0; ch < nchunks; ++ch) {
                     mbar_wait(smem_u32(full + s), ph);
                     tc_fence_after();
-                    const uint32_t b_base = smem_u32(st_ptr + (size_t)s * stage_bytes);
-                    for (int k = 0; k < p.KBS; ++k) {
-                        const int kb = ch * p.KBS + k;
+                    const uint32_t b_lo = b_lo0 + s * stage_step;
+                    if (!skip) {
 #pragma unroll
-                        for (int kk = 0; kk < 4; ++kk) {  // four 32-byte K steps per 128-byte dimension block
-                            const uint64_t bd = umma_desc(b_base + k * KB_TILE_BYTES + kk * 32);
-                            const uint32_t acc = (kb | kk) != 0;
-                            for (int mb = 0; mb < p.MB; ++mb) {
-                                const uint64_t ad = umma_desc(a_base + (mb * p.NKB + kb) * A_BLOCK_BYTES + kk * 32);
-                                tc_mma<TF32>(d_tmem + mb * BN, ad, bd, p.idesc, acc);
+                        for (int k = 0; k < KBS; ++k) {
+#pragma unroll
+                            for (int kk = 0; kk < 4; ++kk) {  // four 32-byte K steps per 128-byte dimension block
+                                const uint64_t bd = ((uint64_t)DESC_HI << 32) | (b_lo + k * (KB_TILE_BYTES >> 4) + kk * 2);
+#pragma unroll
+                                for (int mb = 0; mb < MB; ++mb) {
+                                    const uint64_t ad = ((uint64_t)DESC_HI << 32) |
+                                                        (a_lo + mb * a_mb_step + k * (A_BLOCK_BYTES >> 4) + kk * 2);
+                                    if (k == 0 && kk == 0)
+                                        tc_mma<TF32>(d_tmem + mb * BN, ad, bd, idesc, ch != 0);
+                                    else
+                                        tc_mma<TF32>(d_tmem + mb * BN, ad, bd, idesc, 1u);
+                                }
                             }
                         }
                     }
+                    a_lo += KBS * (A_BLOCK_BYTES >> 4);
                     tc_commit(smem_u32(empty + s));  // frees the smem stage once these MMAs have read it
                     if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
                 }
@@ -397,7 +450,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
         const uint32_t flags = (uint32_t)p.Nq_pad | (row_valid ? 0x100u : 0u) | (writer ? 0x200u : 0u);
         float m = -INFINITY;  // Alg. 3 line 4
 
-        const uint32_t nt = (uint32_t)p.NT, tstride = (uint32_t)(p.MB * BN);
+        const uint32_t nt = (uint32_t)p.NT, tstride = (uint32_t)(MB * BN);
         const uint32_t taddr0 = tmem_base + ((uint32_t)(quad * 32) << 16) + mb * BN;
         uint32_t ts = 0, tph = 0, g = 0, gph = 0;
         for (int64_t t = 0; t < ntiles; ++t) {
@@ -412,39 +465,28 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
             mbar_wait(smem_u32(sfull + g), gph);
             const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
             tmem_ld_wait();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(tempty + ts));  // accumulator stage is free again
             uint32_t k = 0;
             const uint32_t mw[4] = {mask.x, mask.y, mask.z, mask.w};
 #pragma unroll
             for (int c4 = 0; c4 < 4; ++c4) {
-                const uint32_t bits = mw[c4];
-                if (bits == 0) {  // no document ends inside these 32 columns: a max tree, 3 inputs per instruction
-                    const float* x = v + c4 * 32;
-                    float a[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) a[j] = fmaxf(fmaxf(x[4 * j], x[4 * j + 1]), fmaxf(x[4 * j + 2], x[4 * j + 3]));
-                    const float b0 = fmaxf(fmaxf(a[0], a[1]), a[2]), b1 = fmaxf(fmaxf(a[3], a[4]), a[5]);
-                    m = fmaxf(fmaxf(m, b0), fmaxf(fmaxf(b1, a[6]), a[7]));
-                    continue;
-                }
-#pragma unroll
-                for (int ch = 0; ch < 4; ++ch) {
-                    const uint32_t b8 = (bits >> (8 * ch)) & 0xffu;
-                    const float* x = v + c4 * 32 + ch * 8;
-                    if (b8 == 0) {  // no document ends inside these 8 columns
-                        const float m01 = fmaxf(fmaxf(x[0], x[1]), x[2]);
-                        const float m23 = fmaxf(fmaxf(x[3], x[4]), x[5]);
-                        m = fmaxf(fmaxf(m, m01), fmaxf(fmaxf(m23, x[6]), x[7]));
-                    } else {
-                        const uint2 r = epi_boundary_chunk(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], b8, m, k, flags,
-                                                           seg[g].doc, out);
-                        m = __uint_as_float(r.x);
-                        k = r.y;
-                    }
+                const uint32_t bits = (p.debug & 1) ? 0u : mw[c4];
+                if (p.debug & 1) {
+                    m = fmaxf(m, v[c4 * 32]);
+                } else if (bits == 0) {  // no document ends inside these 32 columns
+                    m = max_tree32(m, v + c4 * 32);
+                } else if (bits == 0x80000000u) {  // exactly one document ends, at the last of the 32 columns
+                    epi_flush(max_tree32(m, v + c4 * 32), k, flags, seg[g].doc, out);
+                    ++k;
+                    m = -INFINITY;
+                } else {
+                    const uint2 r = epi_boundary_word(taddr + c4 * 32, bits, m, k, flags, seg[g].doc, out);
+                    m = __uint_as_float(r.x);
+                    k = r.y;
                 }
             }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(tempty + ts));  // accumulator stage is free again
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
             if (++ts == nt) { ts = 0; tph ^= 1; }
@@ -523,6 +565,10 @@ bool plan(const DenseArgs& a, Params& p, uint32_t& smem_bytes) {
     p.NKB = a.d * esize / KB_BYTES;
     p.kb_elems = KB_BYTES / esize;
     p.NT = TMEM_COLS / (p.MB * BN);
+    {
+        const char* dbg = getenv("TMS_DEBUG");
+        p.debug = dbg ? atoi(dbg) : 0;
+    }
     p.KBS = (p.NKB % 2 == 0) ? 2 : 1;
     const uint32_t fmt = a.dtype == TMS_DTYPE_BF16 ? 1u : (a.dtype == TMS_DTYPE_F16 ? 0u : 2u);
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
@@ -567,7 +613,9 @@ int launch_dense_tc(const DenseArgs& a) {
                      (uint32_t)a.Nq))
         return TMS_ERR_CUDA;
 
-    auto kern = dense_tc_kernel<false>;
+    void (*kern)(const CUtensorMap, const CUtensorMap, const Params) = nullptr;
+    if (p.MB == 1) kern = p.KBS == 1 ? dense_tc_kernel<false, 1, 1> : dense_tc_kernel<false, 1, 2>;
+    else kern = p.KBS == 1 ? dense_tc_kernel<false, 2, 1> : dense_tc_kernel<false, 2, 2>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return TMS_ERR_CUDA;
     // no more CTAs than 128-token tiles; one CTA per SM
