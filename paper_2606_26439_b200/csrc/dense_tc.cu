@@ -1,24 +1,28 @@
-// dense_tc.cu -- fused multi-query MaxSim on sm_100a: TMA-fed, tcgen05 tensor cores, TMEM accumulators
-// (TMS_VARIANT_TCGEN05).  Rebuilds the paper's V2-MQ kernel (Alg. 3) and its dimension-tiled
-// form for Blackwell; the Triton/H100 tiling of the paper is prior art, not the blueprint.
+// dense_tc.cu -- fused multi-query MaxSim on sm_100a: TMA-fed, tcgen05 tensor cores, TMEM operands and
+// accumulators (TMS_VARIANT_TCGEN05).  Rebuilds the paper's V2-MQ kernel (Alg. 3) and its
+// dimension-tiled form for Blackwell; the Triton/H100 tiling of the paper is prior art, not the blueprint.
 //
 // Persistent kernel, one CTA per SM.  Each CTA owns a contiguous, token-balanced range of documents cut at
 // document boundaries (no cross-CTA merge, no atomics: the paper's atomic_add of Alg. 3 line 10 is gone).
 //
-//   A operand  Qmat[rows, d]: all Q queries x Nq tokens (Nq padded to a power of two), resident in shared
-//              memory for the whole kernel, K-major, 128-byte swizzle       ("Load Q_tile once", Alg. 3 line 3)
+//   A operand  Qmat[rows, d]: up to 256 query rows (Q queries x Nq tokens, Nq padded to a power of two) resident
+//              in TENSOR MEMORY for the whole kernel ("Load Q_tile once", Alg. 3 line 3).  Each epilogue thread
+//              owns one row and writes it with tcgen05.st; shared memory then only carries document tiles, so
+//              the tensor pipe reads half the shared-memory bytes an SS-mode MMA would.
 //   B operand  128 packed document tokens x (1 or 2) 128-byte dimension blocks per pipeline stage, brought by
-//              TMA exactly once from HBM                                                   (Alg. 3 line 6; Eq. 7)
-//   D          S = Qmat . D_tile^T in TMEM, fp32, one 128-lane x 128-column block per 128 query rows; for
-//              d*sizeof > one stage the MMAs of successive dimension chunks accumulate into the same TMEM
-//              block and the max is taken once after the last chunk
-//   epilogue   tcgen05.ld -> registers; running max per query row, segmented by document with a carry across
-//              tiles (Alg. 3 line 8); at a document's last token the Nq maxima are summed with warp shuffles
-//              and ONE fp32 is stored to scores[q, b]                                        (Eq. 1)
+//              TMA exactly once from HBM, 128-byte swizzle                              (Alg. 3 line 6; Eq. 7)
+//   D          S = Qmat . D_tile^T in TMEM, fp32, one 128-lane x 128-column accumulator per 128 query rows, in
+//              a ring of accumulators.  For d*sizeof > one stage the MMAs of successive dimension chunks
+//              accumulate into the same accumulator; the max is taken once after the last chunk
+//   epilogue   tcgen05.ld (32 columns at a time, the next load in flight while the current columns are
+//              reduced) -> running max per query row, segmented by document with a carry across tiles
+//              (Alg. 3 line 8).  At a document's last token each row parks its maximum in a small per-warp
+//              shared-memory buffer; every 16 documents the warp sums the Nq maxima of each query in ascending
+//              row order and stores 16 scores                                                        (Eq. 1)
 //
 // Warp roles (blockDim = 128 + 128*MB): warp 0 TMA producer, warp 1 MMA issuer + TMEM owner, warp 2 document
 // segmenter (turns `offsets` into per-tile boundary masks, writes -inf for empty documents), warp 3 idle,
-// warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of M-block (w-4)/4).
+// warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of query block (w-4)/4).
 #include <cuda.h>
 #include <cstdlib>
 #include <cuda_runtime.h>
@@ -28,28 +32,32 @@
 namespace tms {
 namespace {
 
-constexpr int BN = 128;            // document tokens per tile (= UMMA N)
-constexpr int KB_BYTES = 128;      // one dimension block: 128 bytes of a row (64 x 16-bit or 32 x fp32)
+constexpr int BN = 128;            // document tokens per tile (= UMMA N) = columns of one accumulator
+constexpr int KB_BYTES = 128;      // one dimension block: 128 bytes of a row (64 x 16-bit)
+constexpr int KB_WORDS = 32;       // ... = 32 TMEM columns of the A operand
 constexpr int KB_TILE_BYTES = BN * KB_BYTES;  // 16 KB: one dimension block of one document tile
-constexpr int A_BLOCK_BYTES = 128 * KB_BYTES; // 16 KB: one dimension block of one 128-row query block
 constexpr int NSEG = 4;            // depth of the segment-info ring
-constexpr int MAX_STAGES = 12;
+constexpr int MAX_STAGES = 14;
+constexpr int MAX_ACC = 4;
 constexpr int TMEM_COLS = 512;
+constexpr int PEND = 32;           // documents parked per epilogue warp before their scores are summed and stored
+constexpr int PEND_PITCH = 33;     // floats per parked document (32 rows + 1: conflict-free column reads)
 constexpr uint32_t SMEM_LIMIT = 232448;  // 227 KB
 
 struct Params {
+    const void* queries;   // this launch's first query
     const int64_t* offsets;
-    float* scores;
+    float* scores;         // this launch's first score row
     int64_t B, T;
-    int Q, Nq, Nq_pad;
-    int MB;        // 128-row query blocks (1 or 2)
-    int NKB;       // dimension blocks per row = d*sizeof/128
-    int KBS;       // dimension blocks per pipeline stage
-    int NS;        // pipeline stages
-    int NT;        // TMEM accumulator stages = 512 / (MB*128)
+    int Q, Nq, Nq_pad;     // queries in this launch
+    int row_bytes;         // d * sizeof(element)
+    int NKB;               // dimension blocks per row = row_bytes / 128
+    int NS;                // pipeline stages
+    int NACC;              // accumulators in the TMEM ring
+    int acc_col0;          // first TMEM column of the ring (the A operand sits in columns [0, MB*NKB*32))
     uint32_t idesc;
-    int kb_elems;  // elements per dimension block (64 or 32)
-    int debug;     // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs
+    int kb_elems;          // elements per dimension block (64)
+    int debug;             // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs
 };
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------
@@ -90,35 +98,27 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
+// true in exactly one lane of the (converged) warp
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.b32 %0, 1, 0, P;\n}\n" : "=r"(pred));
+    return pred != 0;
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-// D[tmem] (+)= A[smem] . B[smem]^T, kind::f16 (fp16/bf16 in, fp32 accumulate) or kind::tf32
-template <bool TF32>
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
-                                       uint32_t accumulate) {
-    if constexpr (TF32) {
-        asm volatile(
-            "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-            "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
-            "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-            : "memory");
-    } else {
-        asm volatile(
-            "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
-            "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-            : "memory");
-    }
+// D[tmem] (+)= A[tmem] . B[smem]^T, kind::f16 (fp16/bf16 in, fp32 accumulate)
+__device__ __forceinline__ void tc_mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                          uint32_t accumulate) {
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n}\n" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
 }
-// 32 lanes x 32 consecutive fp32 columns -> 32 registers per thread (lane l of the warp gets TMEM lane base+l)
+// 32 lanes x 32 consecutive 32-bit columns <-> 32 registers per thread (lane l of the warp owns TMEM lane base+l)
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
     uint32_t* r = reinterpret_cast<uint32_t*>(v);
     asm volatile(
@@ -132,14 +132,40 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
         : "r"(taddr)
         : "memory");
 }
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// K-major, 128-byte-swizzled operand tile: rows of 128 bytes, 8-row groups 1024 bytes apart (SBO),
-// descriptor version 1 (sm_100), layout type 2 (SWIZZLE_128B).  LBO is unused for this layout.
-__device__ __forceinline__ uint64_t umma_desc(uint32_t smem_addr) {
-    return (uint64_t)((smem_addr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) |
-           (2ull << 61);
+// Waits for every tcgen05.ld of this thread.  The 32 registers of the load being waited for pass through the
+// statement as in/out operands so that no use of them can be scheduled above the wait.
+__device__ __forceinline__ void tmem_ld_wait32(float* v) {
+    uint32_t* r = reinterpret_cast<uint32_t*>(v);
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]),
+                   "+r"(r[15]), "+r"(r[16]), "+r"(r[17]), "+r"(r[18]), "+r"(r[19]), "+r"(r[20]), "+r"(r[21]),
+                   "+r"(r[22]), "+r"(r[23]), "+r"(r[24]), "+r"(r[25]), "+r"(r[26]), "+r"(r[27]), "+r"(r[28]),
+                   "+r"(r[29]), "+r"(r[30]), "+r"(r[31])
+                 :
+                 : "memory");
 }
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
+        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
+        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
+__device__ __forceinline__ uint4 ldg_nc16(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+// K-major, 128-byte-swizzled operand tile: rows of 128 bytes, 8-row groups 1024 bytes apart (SBO); descriptor
+// version 1 (sm_100), layout type 2 (SWIZZLE_128B).  LBO is unused for this layout.  High word / constant low bits:
+constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
+constexpr uint32_t DESC_LO = 1u << 16;
 
 // smallest b in [0, B] with offsets[b] >= target; whole warp, 32 probes per round
 __device__ int64_t warp_lower_bound(const int64_t* __restrict__ offsets, int64_t B, int64_t target, int lane) {
@@ -168,105 +194,162 @@ struct SegInfo {
 };
 
 // ---- epilogue helpers ------------------------------------------------------------------------------------------
-// flags: bits 0-7 Nq_pad (a power of two <= 32), bit 8 row holds a real query token, bit 9 row writes the score.
+__device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }  // one FMNMX3
 
-// max -> sum (Eq. 1): the Nq running maxima of one query sit in Nq adjacent lanes; they are summed in a fixed
-// xor-shuffle order and the lane of query token 0 stores the score of the k-th document that ends in this tile.
-__device__ __forceinline__ void flush_inline(float m, uint32_t k, uint32_t flags, const uint32_t* doc, float* out) {
-    const uint32_t nqp = flags & 0xffu;
-    float v = (flags & 0x100u) ? m : 0.f;
-    if (nqp > 16) v += __shfl_xor_sync(0xffffffffu, v, 16);
-    if (nqp > 8) v += __shfl_xor_sync(0xffffffffu, v, 8);
-    if (nqp > 4) v += __shfl_xor_sync(0xffffffffu, v, 4);
-    if (nqp > 2) v += __shfl_xor_sync(0xffffffffu, v, 2);
-    if (nqp > 1) v += __shfl_xor_sync(0xffffffffu, v, 1);
-    if (flags & 0x200u) out[doc[k]] = v;
-}
-__device__ __noinline__ void epi_flush(float m, uint32_t k, uint32_t flags, const uint32_t* doc, float* out) {
-    flush_inline(m, k, flags, doc, out);
+// running max folded with 8 accumulator columns: four 3-input max instructions
+__device__ __forceinline__ float max9(float m, const float* x) {
+    return max3(max3(x[0], x[1], x[2]), max3(x[3], x[4], x[5]), max3(x[6], x[7], m));
 }
 
-// max of 32 accumulator columns and the running max, three inputs per FMNMX3
-__device__ __forceinline__ float max_tree32(float m, const float* x) {
-    float a[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) a[j] = fmaxf(fmaxf(x[4 * j], x[4 * j + 1]), fmaxf(x[4 * j + 2], x[4 * j + 3]));
-    const float b0 = fmaxf(fmaxf(a[0], a[1]), a[2]), b1 = fmaxf(fmaxf(a[3], a[4]), a[5]);
-    return fmaxf(fmaxf(m, b0), fmaxf(fmaxf(b1, a[6]), a[7]));
+// Per-warp constants of the max -> sum step, packed: bits 0-5 Nq, 6-11 Nq_pad, 12-17 queries of this warp that exist.
+__device__ __forceinline__ uint32_t pack_cfg(int Nq, int Nq_pad, int nvalid) {
+    return (uint32_t)Nq | ((uint32_t)Nq_pad << 6) | ((uint32_t)nvalid << 12);
 }
 
-// 32 accumulator columns in which at least one document ends (bit c of `bits`: column c is a document's last token).
-// Out of line and re-reading its columns from TMEM on purpose: boundary words are the minority, and one compact copy
-// of this code keeps the epilogue's hot loop inside the instruction cache.  One iteration per document end: the
-// segment's columns are selected by predicate, folded into the running max, and the document is flushed.
-__device__ __noinline__ uint2 epi_boundary_word(uint32_t taddr, uint32_t bits, float m, uint32_t k, uint32_t flags,
-                                                const uint32_t* doc, float* out) {
-    float x[32];
-    tmem_ld32(taddr, x);
-    tmem_ld_wait();
-    uint32_t done = 0;  // columns that belong to documents already flushed
-    while (bits) {
-        const uint32_t low = bits & (0u - bits);
-        const uint32_t seg = ((low << 1) - 1u) & ~done;
-        float a0 = m, a1 = -INFINITY;
-#pragma unroll
-        for (int c = 0; c < 32; c += 2) {
-            a0 = fmaxf(a0, (seg >> c) & 1u ? x[c] : -INFINITY);
-            a1 = fmaxf(a1, (seg >> (c + 1)) & 1u ? x[c + 1] : -INFINITY);
+// A document's last token has been folded in: row `lane` parks its maximum in slot np of the warp's buffer.
+__device__ __forceinline__ void park(float m, uint32_t k, uint32_t np, float* pend, uint32_t* pend_id,
+                                     const uint32_t* doc, int lane) {
+    pend[np * PEND_PITCH + lane] = m;
+    if (lane == 0) pend_id[np] = doc[k];
+}
+
+// max -> sum (Eq. 1) for the np parked documents: one lane per (document, query of this warp) adds that query's Nq
+// row maxima in ascending row order and stores the score.  Parked documents are consecutive in the usual case, so
+// the stores of a warp coalesce.
+__device__ __noinline__ void drain(float* pend, const uint32_t* pend_id, uint32_t np, float* out, int64_t B,
+                                   uint32_t cfg, int lane) {
+    const uint32_t Nq = cfg & 63u, Nq_pad = (cfg >> 6) & 63u, nvalid = (cfg >> 12) & 63u;
+    const uint32_t nsub = 32u / Nq_pad;
+    __syncwarp();
+    for (uint32_t u = lane; u < np * nsub; u += 32) {
+        const uint32_t slot = u / nsub, sub = u - slot * nsub;
+        if (sub < nvalid) {
+            const float* p = pend + slot * PEND_PITCH + sub * Nq_pad;
+            float acc = p[0];
+            for (uint32_t r = 1; r < Nq; ++r) acc += p[r];
+            out[(int64_t)sub * B + pend_id[slot]] = acc;
         }
-        flush_inline(fmaxf(a0, a1), k, flags, doc, out);
-        ++k;
-        m = -INFINITY;
-        done |= seg;
-        bits ^= low;
     }
-    float a0 = m, a1 = -INFINITY;
-#pragma unroll
-    for (int c = 0; c < 32; c += 2) {
-        a0 = fmaxf(a0, (done >> c) & 1u ? -INFINITY : x[c]);
-        a1 = fmaxf(a1, (done >> (c + 1)) & 1u ? -INFINITY : x[c + 1]);
-    }
-    return make_uint2(__float_as_uint(fmaxf(a0, a1)), k);
+    __syncwarp();
 }
 
-template <bool TF32, int MB, int KBS>
+// running max folded with 32 accumulator columns: sixteen 3-input max instructions, four independent chains
+__device__ __forceinline__ float max33(float m, const float* x) {
+    const float a = max3(max3(x[0], x[1], x[2]), max3(x[3], x[4], x[5]), max3(x[6], x[7], x[8]));
+    const float b = max3(max3(x[9], x[10], x[11]), max3(x[12], x[13], x[14]), max3(x[15], x[16], x[17]));
+    const float c = max3(max3(x[18], x[19], x[20]), max3(x[21], x[22], x[23]), max3(x[24], x[25], x[26]));
+    const float d = max3(max3(x[27], x[28], x[29]), max3(x[30], x[31], m), a);
+    return max3(b, c, d);
+}
+
+struct EpiState {
+    float m;       // running max of this row over the current document's tokens seen so far
+    uint32_t k;    // documents of the current tile already finished
+    uint32_t np;   // documents parked in the warp's buffer
+};
+
+// 32 accumulator columns (copied to local memory by the caller) in which documents end: bit c of `w` marks column
+// c as a document's last token.  Columns are folded in order, 8 at a time, and every finished document is parked.
+// Out of line on purpose: boundary words are the minority, and one compact copy keeps the epilogue's hot loop to
+// a few dozen instructions.  The caller has made sure the park buffer has room.  Returns the new running max.
+__device__ __noinline__ float epi_word_slow(const float* xs, uint32_t w, float m, uint32_t k, uint32_t np, float* pend,
+                                            uint32_t* pend_id, const uint32_t* doc, int lane) {
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        const float4 lo = *reinterpret_cast<const float4*>(xs + 8 * j);
+        const float4 hi = *reinterpret_cast<const float4*>(xs + 8 * j + 4);
+        const float x[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+        const uint32_t byte = (w >> (8 * j)) & 0xffu;
+        if (byte == 0) {
+            m = max9(m, x);
+            continue;
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            m = fmaxf(m, x[c]);
+            if ((byte >> c) & 1u) {
+                park(m, k, np, pend, pend_id, doc, lane);
+                ++k;
+                ++np;
+                m = -INFINITY;  // Alg. 3 line 4 for the next document
+            }
+        }
+    }
+    return m;
+}
+
+// 32 accumulator columns (registers v) with boundary word w.
+__device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, float* pend, uint32_t* pend_id,
+                                          const uint32_t* doc, float* out, int64_t B, uint32_t cfg, int lane,
+                                          bool skip_math) {
+    if (skip_math) {  // measurement probe: TMEM loads without the reduction
+        s.m = fmaxf(s.m, v[0]);
+        return;
+    }
+    if (w == 0) {  // no document ends inside these columns
+        s.m = max33(s.m, v);
+        return;
+    }
+    const uint32_t n = __popc(w);
+    if (s.np + n > PEND) {
+        drain(pend, pend_id, s.np, out, B, cfg, lane);
+        s.np = 0;
+    }
+    if (w == 0x80000000u) {  // one document ends, at the last of the 32 columns
+        park(max33(s.m, v), s.k, s.np, pend, pend_id, doc, lane);
+        s.m = -INFINITY;
+    } else {
+        float xs[32];
+#pragma unroll
+        for (int c = 0; c < 32; ++c) xs[c] = v[c];
+        s.m = epi_word_slow(xs, w, s.m, s.k, s.np, pend, pend_id, doc, lane);
+    }
+    s.k += n;
+    s.np += n;
+}
+
+// KBS: dimension blocks per pipeline stage (2 = a whole 256-byte row block per stage).
+template <int MB, int KBS>
 __global__ void __launch_bounds__(128 + 128 * MB, 1)
-dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_constant__ CUtensorMap map_q,
-                const Params p) {
+dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    // layout: [A: MB*NKB*16 KB] [stages: NS * KBS*16 KB] [SegInfo x NSEG] [barriers] [misc]
-    const uint32_t a_bytes = (uint32_t)MB * p.NKB * A_BLOCK_BYTES;
-    const uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
-    uint8_t* a_ptr = smem;
-    uint8_t* st_ptr = smem + a_bytes;
+    // layout: [stages: NS * KBS*16 KB] [SegInfo x NSEG] [park buffers] [barriers] [misc]
+    constexpr uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
+    constexpr int n_epi_warps = 4 * MB;
+    uint8_t* st_ptr = smem;
     SegInfo* seg = reinterpret_cast<SegInfo*>(st_ptr + (size_t)p.NS * stage_bytes);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(seg + NSEG);
-    // barrier indices
-    uint64_t* full = bars;                       // [NS]
-    uint64_t* empty = full + MAX_STAGES;         // [NS]
-    uint64_t* tfull = empty + MAX_STAGES;        // [4]
-    uint64_t* tempty = tfull + 4;                // [4]
-    uint64_t* sfull = tempty + 4;                // [NSEG]
-    uint64_t* sempty = sfull + NSEG;             // [NSEG]
-    uint64_t* qfull = sempty + NSEG;             // [1]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(qfull + 1);
-    int64_t* range = reinterpret_cast<int64_t*>(qfull + 2);  // b_lo, b_hi, t_lo, t_hi
+    float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps][PEND][PEND_PITCH]
+    uint32_t* pend_id_all = reinterpret_cast<uint32_t*>(pend_all + n_epi_warps * PEND * PEND_PITCH);  // [warps][PEND]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(pend_id_all + n_epi_warps * PEND);
+    uint64_t* full = bars;                       // [NS]   TMA -> MMA
+    uint64_t* empty = full + MAX_STAGES;         // [NS]   MMA -> TMA
+    uint64_t* tdone = empty + MAX_STAGES;        // [4]    MMA -> epilogue: every accumulator of tile t is complete (ring t & 3)
+    uint64_t* tempty = tdone + MAX_ACC;          // [NACC] epilogue -> MMA (4 warps each)
+    uint64_t* sfull = tempty + MAX_ACC;          // [NSEG] segmenter -> epilogue
+    uint64_t* sempty = sfull + NSEG;             // [NSEG] epilogue -> segmenter
+    uint64_t* aready = sempty + NSEG;            // [1]    query rows are in TMEM
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(aready + 1);
+    int64_t* range = reinterpret_cast<int64_t*>(aready + 2);  // b_lo, b_hi, t_lo, t_hi
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_epi_warps = 4 * MB;
+    uint64_t dbg_g0 = 0;
+    long long dbg_c0 = 0;
+    if (p.debug & 8) {
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_g0));
+        dbg_c0 = clock64();
+    }
 
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0) {
         if (lane == 0) {
             for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), 1); mbar_init(smem_u32(empty + s), 1); }
-            for (int s = 0; s < 4; ++s) { mbar_init(smem_u32(tfull + s), 1); mbar_init(smem_u32(tempty + s), n_epi_warps); }
+            for (int s = 0; s < MAX_ACC; ++s) { mbar_init(smem_u32(tdone + s), 1); mbar_init(smem_u32(tempty + s), 4); }
             for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), n_epi_warps); }
-            mbar_init(smem_u32(qfull), 1);
+            mbar_init(smem_u32(aready), n_epi_warps);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&map_q) : "memory");
         }
         // work partition (a3): documents [b_lo, b_hi) whose first tokens lie in [c*T/G, (c+1)*T/G)
         const int64_t G = gridDim.x, c = blockIdx.x;
@@ -284,12 +367,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
                      "r"((uint32_t)TMEM_COLS)
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    } else {
-        // zero the A operand so rows that no query owns are finite (they never reach a score)
-        const int nthr = blockDim.x - 64;
-        uint4* a4 = reinterpret_cast<uint4*>(a_ptr);
-        for (uint32_t i = threadIdx.x - 64; i < a_bytes / 16; i += nthr) a4[i] = make_uint4(0, 0, 0, 0);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy zeros before TMA writes
     }
     tc_fence_before();
     __syncthreads();
@@ -302,84 +379,90 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
 
     if (warp == 0) {
         // ===== TMA producer =====
-        if (lane == 0) {
-            const uint64_t pol_docs = policy_evict_first();  // streamed once
-            const uint64_t pol_q = policy_evict_last();      // every CTA reads the same queries
-            // queries: one box of Nq rows x 128 bytes per (query, dimension block)
-            mbar_expect_tx(smem_u32(qfull), (uint32_t)p.Q * p.Nq * KB_BYTES * p.NKB);
-            for (int q = 0; q < p.Q; ++q) {
-                const int row0 = q * p.Nq_pad;
-                const int mb = row0 >> 7, r = row0 & 127;
-                for (int kb = 0; kb < p.NKB; ++kb)
-                    tma_load_2d(smem_u32(a_ptr + (size_t)(mb * p.NKB + kb) * A_BLOCK_BYTES + r * KB_BYTES), &map_q,
-                                smem_u32(qfull), kb * p.kb_elems, q * p.Nq, pol_q);
-            }
-            uint32_t s = 0, ph = 0;  // ring slot and its phase bit
-            for (int64_t t = 0; t < ntiles; ++t) {
-                const int tok = (int)(t_lo + t * BN);
-                for (int ch = 0; ch < nchunks; ++ch) {
-                    mbar_wait(smem_u32(empty + s), ph ^ 1);
+        // The whole warp runs the loop and waits on the barriers; one elected lane issues the copies, so that the
+        // compiler emits the uniform-datapath instructions straight-line (no per-active-thread loop).
+        const uint64_t pol_docs = policy_evict_first();  // streamed once
+        uint32_t s = 0, ph = 0;  // ring slot and its phase bit
+        for (int64_t t = 0; t < ntiles; ++t) {
+            const int tok = (int)(t_lo + t * BN);
+            for (int ch = 0; ch < nchunks; ++ch) {
+                mbar_wait(smem_u32(empty + s), ph ^ 1);
+                if (elect_one()) {
                     mbar_expect_tx(smem_u32(full + s), stage_bytes);
+#pragma unroll
                     for (int k = 0; k < KBS; ++k)
                         tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
                                     smem_u32(full + s), (ch * KBS + k) * p.kb_elems, tok, pol_docs);
-                    if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
                 }
+                __syncwarp();
+                if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
             }
         }
-        __syncwarp();
     } else if (warp == 1) {
         // ===== MMA issuer =====
-        // One thread issues every tcgen05.mma of the CTA, so its instruction stream must stay short: the loops
-        // over K steps and query blocks are compile-time, and a descriptor is the previous one plus a constant.
-        if (lane == 0) {
-            mbar_wait(smem_u32(qfull), 0);
-            tc_fence_after();
-            constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);  // SBO 1024 B, version 1, SWIZZLE_128B
-            constexpr uint32_t DESC_LO = 1u << 16;                                // LBO field (unused for this layout)
-            const uint32_t a_lo0 = ((smem_u32(a_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
-            const uint32_t a_mb_step = (uint32_t)p.NKB * (A_BLOCK_BYTES >> 4);    // next 128-row query block
-            const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
-            const uint32_t stage_step = stage_bytes >> 4;
-            const uint32_t idesc = p.idesc;
-            const bool skip = (p.debug & 2) != 0;
-            uint32_t s = 0, ph = 0, ts = 0, tph = 0;
-            for (int64_t t = 0; t < ntiles; ++t) {
-                mbar_wait(smem_u32(tempty + ts), tph ^ 1);  // epilogue has drained this accumulator stage
+        // One elected lane issues every tcgen05.mma of the CTA (the whole warp follows the barriers), so its
+        // instruction stream must stay short: the loops over K steps and query blocks are compile-time, and a
+        // descriptor is the previous one plus a constant.
+        mbar_wait(smem_u32(aready), 0);
+        tc_fence_after();
+        const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
+        const uint32_t idesc = p.idesc;
+        const bool skip = (p.debug & 2) != 0;
+        const uint32_t nacc = (uint32_t)p.NACC;
+        const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
+        const uint32_t a_mb_step = (uint32_t)p.NKB * KB_WORDS;  // TMEM columns of one query block's rows
+        uint32_t s = 0, ph = 0;
+        uint32_t slot[MB], tph[MB];
+#pragma unroll
+        for (int mb = 0; mb < MB; ++mb) { slot[mb] = mb; tph[mb] = 0; }
+        for (int64_t t = 0; t < ntiles; ++t) {
+            uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
+            for (int ch = 0; ch < nchunks; ++ch) {
+                mbar_wait(smem_u32(full + s), ph);
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + ts * (uint32_t)(MB * BN);
-                uint32_t a_lo = a_lo0;
-                for (int ch = 0; ch < nchunks; ++ch) {
-                    mbar_wait(smem_u32(full + s), ph);
-                    tc_fence_after();
-                    const uint32_t b_lo = b_lo0 + s * stage_step;
-                    if (!skip) {
+                const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
 #pragma unroll
-                        for (int k = 0; k < KBS; ++k) {
+                for (int mb = 0; mb < MB; ++mb) {
+                    if (ch == 0) {  // the epilogue has drained this accumulator
+                        mbar_wait(smem_u32(tempty + slot[mb]), tph[mb] ^ 1);
+                        tc_fence_after();
+                    }
+                    const uint32_t d_tmem = acc0 + slot[mb] * BN;
+                    if (elect_one()) {
+                        if (!skip) {
 #pragma unroll
-                            for (int kk = 0; kk < 4; ++kk) {  // four 32-byte K steps per 128-byte dimension block
-                                const uint64_t bd = ((uint64_t)DESC_HI << 32) | (b_lo + k * (KB_TILE_BYTES >> 4) + kk * 2);
+                            for (int k = 0; k < KBS; ++k) {
 #pragma unroll
-                                for (int mb = 0; mb < MB; ++mb) {
-                                    const uint64_t ad = ((uint64_t)DESC_HI << 32) |
-                                                        (a_lo + mb * a_mb_step + k * (A_BLOCK_BYTES >> 4) + kk * 2);
+                                for (int kk = 0; kk < 4; ++kk) {  // four 32-byte K steps per 128-byte dimension block
+                                    const uint64_t bd =
+                                        ((uint64_t)DESC_HI << 32) | (b_lo + k * (KB_TILE_BYTES >> 4) + kk * 2);
+                                    const uint32_t at = a_col + mb * a_mb_step + k * KB_WORDS + kk * 8;
                                     if (k == 0 && kk == 0)
-                                        tc_mma<TF32>(d_tmem + mb * BN, ad, bd, idesc, ch != 0);
+                                        tc_mma_ts(d_tmem, at, bd, idesc, ch != 0);
                                     else
-                                        tc_mma<TF32>(d_tmem + mb * BN, ad, bd, idesc, 1u);
+                                        tc_mma_ts(d_tmem, at, bd, idesc, 1u);
                                 }
                             }
                         }
+                        if (mb == MB - 1) {
+                            // One commit per tile when a tile is one stage: "tile done" tells the epilogue that the
+                            // accumulators are complete AND that the stage has been read (an epilogue warp hands the
+                            // stage back to the producer).  Each tcgen05.commit costs the tensor pipe a bubble.
+                            if (ch == nchunks - 1) tc_commit(smem_u32(tdone + (uint32_t)(t & 3)));
+                            if (nchunks > 1) tc_commit(smem_u32(empty + s));
+                        }
                     }
-                    a_lo += KBS * (A_BLOCK_BYTES >> 4);
-                    tc_commit(smem_u32(empty + s));  // frees the smem stage once these MMAs have read it
-                    if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
+                    __syncwarp();
                 }
-                tc_commit(smem_u32(tfull + ts));     // accumulator stage complete -> epilogue
-                if (++ts == (uint32_t)p.NT) { ts = 0; tph ^= 1; }
+                a_col += KBS * KB_WORDS;
+                if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
+            }
+#pragma unroll
+            for (int mb = 0; mb < MB; ++mb) {
+                slot[mb] += MB;
+                if (slot[mb] >= nacc) { slot[mb] -= nacc; tph[mb] ^= 1; }
             }
         }
-        __syncwarp();
     } else if (warp == 2) {
         // ===== document segmenter =====
         // Lane l holds the end offset of document wb + l (a 32-document window in registers); the next window is
@@ -442,61 +525,106 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const __grid_const
     } else if (warp >= 4) {
         // ===== epilogue: running rowmax, segmented by document; max -> sum =====
         const int ew = warp - 4, mb = ew >> 2, quad = warp & 3;
-        const int row = mb * 128 + quad * 32 + lane;
+        const int row = mb * 128 + quad * 32 + lane;   // this thread's query row = TMEM lane quad*32+lane of block mb
         const int q = row / p.Nq_pad, i = row - q * p.Nq_pad;
-        const bool row_valid = (q < p.Q) && (i < p.Nq);
-        const bool writer = row_valid && (i == 0);
-        float* out = p.scores + (int64_t)(q < p.Q ? q : 0) * p.B + b_lo;
-        const uint32_t flags = (uint32_t)p.Nq_pad | (row_valid ? 0x100u : 0u) | (writer ? 0x200u : 0u);
-        float m = -INFINITY;  // Alg. 3 line 4
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(quad * 32) << 16);
 
-        const uint32_t nt = (uint32_t)p.NT, tstride = (uint32_t)(MB * BN);
-        const uint32_t taddr0 = tmem_base + ((uint32_t)(quad * 32) << 16) + mb * BN;
-        uint32_t ts = 0, tph = 0, g = 0, gph = 0;
-        for (int64_t t = 0; t < ntiles; ++t) {
-            mbar_wait(smem_u32(tfull + ts), tph);
-            tc_fence_after();
-            const uint32_t taddr = taddr0 + ts * tstride;
-            float v[BN];
-            tmem_ld32(taddr + 0, v + 0);
-            tmem_ld32(taddr + 32, v + 32);
-            tmem_ld32(taddr + 64, v + 64);
-            tmem_ld32(taddr + 96, v + 96);
-            mbar_wait(smem_u32(sfull + g), gph);
-            const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
-            tmem_ld_wait();
-            uint32_t k = 0;
-            const uint32_t mw[4] = {mask.x, mask.y, mask.z, mask.w};
+        // a2: the thread's query row -> TMEM columns [mb*NKB*32, +NKB*32), two 16-bit elements per column;
+        // rows no query token owns are zero (finite similarities that never reach a score, A5)
+        {
+            const bool row_valid = (q < p.Q) && (i < p.Nq);
+            const uint8_t* src = static_cast<const uint8_t*>(p.queries) + ((int64_t)q * p.Nq + i) * p.row_bytes;
+            for (int kb = 0; kb < p.NKB; ++kb) {
+                uint32_t w[KB_WORDS];
 #pragma unroll
-            for (int c4 = 0; c4 < 4; ++c4) {
-                const uint32_t bits = (p.debug & 1) ? 0u : mw[c4];
-                if (p.debug & 1) {
-                    m = fmaxf(m, v[c4 * 32]);
-                } else if (bits == 0) {  // no document ends inside these 32 columns
-                    m = max_tree32(m, v + c4 * 32);
-                } else if (bits == 0x80000000u) {  // exactly one document ends, at the last of the 32 columns
-                    epi_flush(max_tree32(m, v + c4 * 32), k, flags, seg[g].doc, out);
-                    ++k;
-                    m = -INFINITY;
-                } else {
-                    const uint2 r = epi_boundary_word(taddr + c4 * 32, bits, m, k, flags, seg[g].doc, out);
-                    m = __uint_as_float(r.x);
-                    k = r.y;
+                for (int j = 0; j < KB_WORDS / 4; ++j) {
+                    uint4 x = make_uint4(0, 0, 0, 0);
+                    if (row_valid) x = ldg_nc16(src + kb * KB_BYTES + j * 16);
+                    w[4 * j] = x.x; w[4 * j + 1] = x.y; w[4 * j + 2] = x.z; w[4 * j + 3] = x.w;
                 }
+                tmem_st32(lane_addr + (uint32_t)((mb * p.NKB + kb) * KB_WORDS), w);
             }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(tempty + ts));  // accumulator stage is free again
+            if (lane == 0) mbar_arrive(smem_u32(aready));
+        }
+
+        // max -> sum constants of this warp: its 32 rows hold 32/Nq_pad queries, the first one being q0
+        const int q0 = (mb * 128 + quad * 32) / p.Nq_pad;
+        const int nsub = 32 / p.Nq_pad;
+        const int nvalid = p.Q - q0 < 0 ? 0 : (p.Q - q0 < nsub ? p.Q - q0 : nsub);
+        const uint32_t cfg = pack_cfg(p.Nq, p.Nq_pad, nvalid);
+        float* out = p.scores + (int64_t)q0 * p.B + b_lo;
+        float* pend = pend_all + ew * PEND * PEND_PITCH;
+        uint32_t* pend_id = pend_id_all + ew * PEND;
+        const bool skip_math = (p.debug & 1) != 0;
+        const int64_t B = p.B;
+
+        EpiState st;
+        st.m = -INFINITY;  // Alg. 3 line 4
+        st.k = 0;
+        st.np = 0;
+        const uint32_t nacc = (uint32_t)p.NACC;
+        const uint32_t acc0 = lane_addr + (uint32_t)p.acc_col0;
+        uint32_t slot = (uint32_t)mb, tph = 0, g = 0, gph = 0, rs = 0;
+        for (int64_t t = 0; t < ntiles; ++t) {
+            mbar_wait(smem_u32(tdone + (uint32_t)(t & 3)), (uint32_t)(t >> 2) & 1u);
+            tc_fence_after();
+            if (nchunks == 1 && ew == 0) {  // the tile's only stage has been read by the tensor pipe: back to the producer
+                if (lane == 0) mbar_arrive(smem_u32(empty + rs));
+                if (++rs == (uint32_t)p.NS) rs = 0;
+            }
+            const uint32_t taddr = acc0 + slot * BN;
+            float va[32], vb[32];
+            if (p.debug & 4) {  // measurement probe: no TMEM reads at all
+                mbar_wait(smem_u32(sfull + g), gph);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(smem_u32(tempty + slot)); mbar_arrive(smem_u32(sempty + g)); }
+                slot += MB;
+                if (slot >= nacc) { slot -= nacc; tph ^= 1; }
+                if (++g == NSEG) { g = 0; gph ^= 1; }
+                continue;
+            }
+            tmem_ld32(taddr, va);
+            mbar_wait(smem_u32(sfull + g), gph);
+            const uint32_t* doc = seg[g].doc;
+            const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
+            st.k = 0;
+            tmem_ld_wait32(va);
+            tmem_ld32(taddr + 32, vb);  // in flight while columns 0..31 are reduced
+            process32(va, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            tmem_ld_wait32(vb);
+            tmem_ld32(taddr + 64, va);
+            process32(vb, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            tmem_ld_wait32(va);
+            tmem_ld32(taddr + 96, vb);
+            process32(va, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            tmem_ld_wait32(vb);
+            // every column is in registers: hand the accumulator back before reducing the last 32
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
+            process32(vb, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
-            if (++ts == nt) { ts = 0; tph ^= 1; }
+            slot += MB;
+            if (slot >= nacc) { slot -= nacc; tph ^= 1; }
             if (++g == NSEG) { g = 0; gph ^= 1; }
         }
+        if (st.np) drain(pend, pend_id, st.np, out, B, cfg, lane);
     }
 
     // ---- teardown --------------------------------------------------------------------------------------------
     tc_fence_before();
     __syncthreads();
+    if ((p.debug & 8) && threadIdx.x == 0) {  // measurement probe: SM clock seen by this CTA (overwrites two scores)
+        uint64_t g1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+        p.scores[2 * blockIdx.x] = (float)(clock64() - dbg_c0);
+        p.scores[2 * blockIdx.x + 1] = (float)(g1 - dbg_g0);
+    }
     if (warp == 1) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)TMEM_COLS)
@@ -543,50 +671,65 @@ int next_pow2(int v) {
     return p;
 }
 
+struct Plan {
+    Params p;           // per-launch fields (queries, scores, Q) are filled in by the launcher
+    int MB, KBS;        // query blocks per launch, dimension blocks per stage
+    int Qg;             // queries per launch
+    uint32_t smem_bytes;
+};
+
+uint32_t fixed_smem(int MB) {
+    const uint32_t warps = 4u * MB;
+    return (uint32_t)sizeof(SegInfo) * NSEG + warps * PEND * (PEND_PITCH + 1) * 4 +
+           8u * (2 * MAX_STAGES + 2 * MAX_ACC + 2 * NSEG + 2) + 4 * 8 + 1024 /* alignment slack */;
+}
+
 // Shape -> kernel parameters; false when the tcgen05 path does not cover it.
-bool plan(const DenseArgs& a, Params& p, uint32_t& smem_bytes) {
+bool plan(const DenseArgs& a, Plan& pl) {
     if (a.B <= 0 || a.T <= 0 || a.T >= (1ll << 31) - BN) return false;
     if (a.dtype == TMS_DTYPE_F32) return false;  // fp32 inputs: plain TF32 would break the 1e-5*Nq tolerance
     const int esize = (int)dtype_size(a.dtype);
-    if ((a.d * esize) % KB_BYTES != 0) return false;
+    const int row_bytes = a.d * esize;
+    if (row_bytes % KB_BYTES != 0) return false;
     const int nqp = next_pow2(a.Nq);
-    if (nqp > 32) return false;
-    const int nqp8 = nqp < 8 ? 8 : nqp;  // query blocks start on 8-row (1024-byte) swizzle-atom boundaries
-    const int rows = a.Q * nqp8;
-    if (rows > 256) return false;
+    if (nqp > 32) return false;  // a query's rows must sit inside one warp's 32 TMEM lanes
+    const int NKB = row_bytes / KB_BYTES;
+    // TMEM budget: MB*NKB*32 columns of query rows + at least MB accumulators of 128 columns
+    int MB = 2;
+    if (MB * NKB * KB_WORDS + MB * BN > TMEM_COLS) MB = 1;
+    if (MB * NKB * KB_WORDS + MB * BN > TMEM_COLS) return false;  // d too large for a resident query block
+    const int per_block = 128 / nqp;  // queries per 128-row block
+    if (a.Q <= per_block) MB = 1;
+    Params& p = pl.p;
     p.offsets = a.offsets;
-    p.scores = a.scores;
     p.B = a.B;
     p.T = a.T;
-    p.Q = a.Q;
     p.Nq = a.Nq;
-    p.Nq_pad = nqp8;
-    p.MB = (rows + 127) / 128;
-    p.NKB = a.d * esize / KB_BYTES;
+    p.Nq_pad = nqp;
+    p.row_bytes = row_bytes;
+    p.NKB = NKB;
     p.kb_elems = KB_BYTES / esize;
-    p.NT = TMEM_COLS / (p.MB * BN);
+    const int a_cols = MB * NKB * KB_WORDS;
+    p.NACC = (TMEM_COLS - a_cols) / BN;
+    if (p.NACC > MAX_ACC) p.NACC = MAX_ACC;
+    p.acc_col0 = TMEM_COLS - p.NACC * BN;
     {
         const char* dbg = getenv("TMS_DEBUG");
         p.debug = dbg ? atoi(dbg) : 0;
     }
-    p.KBS = (p.NKB % 2 == 0) ? 2 : 1;
-    const uint32_t fmt = a.dtype == TMS_DTYPE_BF16 ? 1u : (a.dtype == TMS_DTYPE_F16 ? 0u : 2u);
+    const uint32_t fmt = a.dtype == TMS_DTYPE_BF16 ? 1u : 0u;
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-    const uint32_t a_bytes = (uint32_t)p.MB * p.NKB * A_BLOCK_BYTES;
-    const uint32_t fixed = sizeof(SegInfo) * NSEG + 8 * (2 * MAX_STAGES + 8 + 2 * NSEG + 2) + 4 * 8 + 1024;
-    if (a_bytes + fixed + 2u * KB_TILE_BYTES > SMEM_LIMIT) return false;
-    uint32_t stage_bytes = (uint32_t)p.KBS * KB_TILE_BYTES;
-    int ns = (int)((SMEM_LIMIT - a_bytes - fixed) / stage_bytes);
-    if (ns < 3 && p.KBS == 2) {  // fall back to 16 KB stages when the resident queries leave little room
-        p.KBS = 1;
-        stage_bytes = KB_TILE_BYTES;
-        ns = (int)((SMEM_LIMIT - a_bytes - fixed) / stage_bytes);
-    }
-    if (ns < 2) return false;
+    pl.MB = MB;
+    pl.Qg = MB * per_block;
+    pl.KBS = (NKB % 2 == 0) ? 2 : 1;
+    const uint32_t fixed = fixed_smem(MB);
+    const uint32_t stage_bytes = (uint32_t)pl.KBS * KB_TILE_BYTES;
+    int ns = (int)((SMEM_LIMIT - fixed) / stage_bytes);
     p.NS = ns > MAX_STAGES ? MAX_STAGES : ns;
-    smem_bytes = a_bytes + (uint32_t)p.NS * stage_bytes + fixed;
-    return true;
+    if (const char* e = getenv("TMS_NS")) { int v = atoi(e); if (v >= 2 && v < p.NS) p.NS = v; }
+    pl.smem_bytes = (uint32_t)p.NS * stage_bytes + fixed;
+    return p.NS >= 2;
 }
 
 }  // namespace
@@ -594,36 +737,39 @@ bool plan(const DenseArgs& a, Params& p, uint32_t& smem_bytes) {
 bool dense_tc_supports(const DenseArgs& a) {
     const DeviceInfo* di = device_info();
     if (!di || di->cc_major != 10) return false;
-    Params p;
-    uint32_t smem;
-    return plan(a, p, smem) && smem <= (uint32_t)di->max_smem_optin;
+    Plan pl;
+    return plan(a, pl) && pl.smem_bytes <= (uint32_t)di->max_smem_optin;
 }
 
 int launch_dense_tc(const DenseArgs& a) {
     const DeviceInfo* di = device_info();
     if (!di) return TMS_ERR_CUDA;
-    Params p;
-    uint32_t smem = 0;
-    if (di->cc_major != 10 || !plan(a, p, smem) || smem > (uint32_t)di->max_smem_optin) return TMS_ERR_UNSUPPORTED;
+    Plan pl;
+    if (di->cc_major != 10 || !plan(a, pl) || pl.smem_bytes > (uint32_t)di->max_smem_optin) return TMS_ERR_UNSUPPORTED;
 
-    CUtensorMap map_docs, map_q;
-    if (!make_map_2d(&map_docs, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d, (uint32_t)p.kb_elems, BN))
-        return TMS_ERR_CUDA;
-    if (!make_map_2d(&map_q, a.dtype, a.queries, (uint64_t)a.Q * a.Nq, (uint64_t)a.d, (uint32_t)p.kb_elems,
-                     (uint32_t)a.Nq))
+    CUtensorMap map_docs;
+    if (!make_map_2d(&map_docs, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d, (uint32_t)pl.p.kb_elems, BN))
         return TMS_ERR_CUDA;
 
-    void (*kern)(const CUtensorMap, const CUtensorMap, const Params) = nullptr;
-    if (p.MB == 1) kern = p.KBS == 1 ? dense_tc_kernel<false, 1, 1> : dense_tc_kernel<false, 1, 2>;
-    else kern = p.KBS == 1 ? dense_tc_kernel<false, 2, 1> : dense_tc_kernel<false, 2, 2>;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    void (*kern)(const CUtensorMap, const Params) = nullptr;
+    if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1> : dense_tc_kernel<1, 2>;
+    else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1> : dense_tc_kernel<2, 2>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess)
         return TMS_ERR_CUDA;
     // no more CTAs than 128-token tiles; one CTA per SM
     int64_t grid = (a.T + BN - 1) / BN;
     if (grid > di->num_sms) grid = di->num_sms;
-    kern<<<(unsigned)grid, 128 + 128 * p.MB, smem, a.stream>>>(map_docs, map_q, p);
-    count_launch();
-    return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
+    // one launch per group of Qg queries (up to 256 query rows): the store is streamed once per group
+    for (int q0 = 0; q0 < a.Q; q0 += pl.Qg) {
+        Params p = pl.p;
+        p.Q = a.Q - q0 < pl.Qg ? a.Q - q0 : pl.Qg;
+        p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * a.Nq * p.row_bytes;
+        p.scores = a.scores + (int64_t)q0 * a.B;
+        kern<<<(unsigned)grid, 128 + 128 * pl.MB, pl.smem_bytes, a.stream>>>(map_docs, p);
+        count_launch();
+        if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+    }
+    return TMS_OK;
 }
 
 }  // namespace tms
