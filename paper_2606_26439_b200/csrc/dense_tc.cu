@@ -40,7 +40,7 @@ constexpr int NSEG = 4;            // depth of the segment-info ring
 constexpr int MAX_STAGES = 14;
 constexpr int MAX_ACC = 4;
 constexpr int TMEM_COLS = 512;
-constexpr int PEND = 32;           // documents parked per epilogue warp before their scores are summed and stored
+constexpr int PEND = 16;           // documents parked per epilogue warp before their scores are summed and stored
 constexpr int PEND_PITCH = 33;     // floats per parked document (32 rows + 1: conflict-free column reads)
 constexpr uint32_t SMEM_LIMIT = 232448;  // 227 KB
 
@@ -145,6 +145,18 @@ __device__ __forceinline__ void tmem_ld_wait32(float* v) {
                  :
                  : "memory");
 }
+// No instruction: makes later uses of these 32 registers depend on a statement that follows the wait above.
+__device__ __forceinline__ void tmem_ld_pin32(float* v) {
+    uint32_t* r = reinterpret_cast<uint32_t*>(v);
+    asm volatile(""
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                   "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]),
+                   "+r"(r[15]), "+r"(r[16]), "+r"(r[17]), "+r"(r[18]), "+r"(r[19]), "+r"(r[20]), "+r"(r[21]),
+                   "+r"(r[22]), "+r"(r[23]), "+r"(r[24]), "+r"(r[25]), "+r"(r[26]), "+r"(r[27]), "+r"(r[28]),
+                   "+r"(r[29]), "+r"(r[30]), "+r"(r[31])
+                 :
+                 : "memory");
+}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
@@ -225,9 +237,14 @@ __device__ __noinline__ void drain(float* pend, const uint32_t* pend_id, uint32_
         const uint32_t slot = u / nsub, sub = u - slot * nsub;
         if (sub < nvalid) {
             const float* p = pend + slot * PEND_PITCH + sub * Nq_pad;
-            float acc = p[0];
-            for (uint32_t r = 1; r < Nq; ++r) acc += p[r];
-            out[(int64_t)sub * B + pend_id[slot]] = acc;
+            // all loads first (independent), then four partial sums over rows r = 0,4,8.. / 1,5,.. / 2,6,.. / 3,7,..
+            float x[32];
+#pragma unroll
+            for (int r = 0; r < 32; ++r) x[r] = (uint32_t)r < Nq ? p[r] : 0.f;
+            float a0 = x[0], a1 = x[1], a2 = x[2], a3 = x[3];
+#pragma unroll
+            for (int r = 4; r < 32; r += 4) { a0 += x[r]; a1 += x[r + 1]; a2 += x[r + 2]; a3 += x[r + 3]; }
+            out[(int64_t)sub * B + pend_id[slot]] = (a0 + a1) + (a2 + a3);
         }
     }
     __syncwarp();
@@ -248,37 +265,29 @@ struct EpiState {
     uint32_t np;   // documents parked in the warp's buffer
 };
 
-// 32 accumulator columns (copied to local memory by the caller) in which documents end: bit c of `w` marks column
-// c as a document's last token.  Columns are folded in order, 8 at a time, and every finished document is parked.
-// Out of line on purpose: boundary words are the minority, and one compact copy keeps the epilogue's hot loop to
-// a few dozen instructions.  The caller has made sure the park buffer has room.  Returns the new running max.
-__device__ __noinline__ float epi_word_slow(const float* xs, uint32_t w, float m, uint32_t k, uint32_t np, float* pend,
-                                            uint32_t* pend_id, const uint32_t* doc, int lane) {
-#pragma unroll 1
-    for (int j = 0; j < 4; ++j) {
-        const float4 lo = *reinterpret_cast<const float4*>(xs + 8 * j);
-        const float4 hi = *reinterpret_cast<const float4*>(xs + 8 * j + 4);
-        const float x[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
-        const uint32_t byte = (w >> (8 * j)) & 0xffu;
-        if (byte == 0) {
-            m = max9(m, x);
-            continue;
-        }
+// 8 accumulator columns in which documents end (bit c of `byte`: column c is a document's last token): columns
+// are folded in order and every finished document is parked.  Out of line: boundary chunks are the minority, and
+// one compact copy keeps the epilogue's hot loop short.  The caller has made sure the buffer has room.
+__device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float x3, float x4, float x5, float x6,
+                                             float x7, uint32_t byte, float m, uint32_t k, uint32_t np, float* pend,
+                                             uint32_t* pend_id, const uint32_t* doc, int lane) {
+    const float x[8] = {x0, x1, x2, x3, x4, x5, x6, x7};
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            m = fmaxf(m, x[c]);
-            if ((byte >> c) & 1u) {
-                park(m, k, np, pend, pend_id, doc, lane);
-                ++k;
-                ++np;
-                m = -INFINITY;  // Alg. 3 line 4 for the next document
-            }
+    for (int c = 0; c < 8; ++c) {
+        m = fmaxf(m, x[c]);
+        if (byte & (1u << c)) {
+            park(m, k, np, pend, pend_id, doc, lane);
+            ++k;
+            ++np;
+            m = -INFINITY;  // Alg. 3 line 4 for the next document
         }
     }
     return m;
 }
 
-// 32 accumulator columns (registers v) with boundary word w.
+// 32 accumulator columns (registers v) with boundary word w: bit c set = column c is a document's last token.
+// Words without a boundary (the majority) take sixteen 3-input max instructions, and so does a word whose only
+// boundary is its last column (uniform 128-token documents).  Otherwise the word is walked in 8-column chunks.
 __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, float* pend, uint32_t* pend_id,
                                           const uint32_t* doc, float* out, int64_t B, uint32_t cfg, int lane,
                                           bool skip_math) {
@@ -286,26 +295,56 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
         s.m = fmaxf(s.m, v[0]);
         return;
     }
-    if (w == 0) {  // no document ends inside these columns
+    if (w == 0) {
         s.m = max33(s.m, v);
         return;
     }
-    const uint32_t n = __popc(w);
-    if (s.np + n > PEND) {
-        drain(pend, pend_id, s.np, out, B, cfg, lane);
-        s.np = 0;
-    }
-    if (w == 0x80000000u) {  // one document ends, at the last of the 32 columns
+    if (w == 0x80000000u) {
+        if (s.np == PEND) {
+            drain(pend, pend_id, s.np, out, B, cfg, lane);
+            s.np = 0;
+        }
         park(max33(s.m, v), s.k, s.np, pend, pend_id, doc, lane);
+        ++s.k;
+        ++s.np;
         s.m = -INFINITY;
-    } else {
-        float xs[32];
-#pragma unroll
-        for (int c = 0; c < 32; ++c) xs[c] = v[c];
-        s.m = epi_word_slow(xs, w, s.m, s.k, s.np, pend, pend_id, doc, lane);
+        return;
     }
-    s.k += n;
-    s.np += n;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t byte = (w >> (8 * j)) & 0xffu;
+        const float* x = v + 8 * j;
+        if (byte == 0) {
+            s.m = max9(s.m, x);
+            continue;
+        }
+        if (s.np + 8 > PEND) {  // room for the up to 8 documents that may end in this chunk
+            drain(pend, pend_id, s.np, out, B, cfg, lane);
+            s.np = 0;
+        }
+        if ((byte & (byte - 1)) == 0) {
+            // exactly one document ends in this chunk, at column e: branch-free split into the columns up to e (they
+            // close the document) and the columns after e (they open the next one)
+            const int e = 31 - __clz((int)byte);
+            float l[8], r[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const bool left = e >= c;
+                l[c] = left ? x[c] : -INFINITY;
+                r[c] = left ? -INFINITY : x[c];
+            }
+            park(max9(s.m, l), s.k, s.np, pend, pend_id, doc, lane);
+            s.m = max9(-INFINITY, r);  // Alg. 3 line 4 for the next document, then its first columns
+            ++s.k;
+            ++s.np;
+        } else {
+            s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.k, s.np, pend, pend_id,
+                                 doc, lane);
+            const uint32_t n = __popc(byte);
+            s.k += n;
+            s.np += n;
+        }
+    }
 }
 
 // KBS: dimension blocks per pipeline stage (2 = a whole 256-byte row block per stage).
@@ -418,12 +457,12 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         for (int64_t t = 0; t < ntiles; ++t) {
             uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
             for (int ch = 0; ch < nchunks; ++ch) {
-                mbar_wait(smem_u32(full + s), ph);
+                if (!(p.debug & 32)) mbar_wait(smem_u32(full + s), ph);
                 tc_fence_after();
                 const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
 #pragma unroll
                 for (int mb = 0; mb < MB; ++mb) {
-                    if (ch == 0) {  // the epilogue has drained this accumulator
+                    if (ch == 0 && !(p.debug & 16)) {  // the epilogue has drained this accumulator
                         mbar_wait(smem_u32(tempty + slot[mb]), tph[mb] ^ 1);
                         tc_fence_after();
                     }
@@ -576,7 +615,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 if (++rs == (uint32_t)p.NS) rs = 0;
             }
             const uint32_t taddr = acc0 + slot * BN;
-            float va[32], vb[32];
+            float v[BN];
             if (p.debug & 4) {  // measurement probe: no TMEM reads at all
                 mbar_wait(smem_u32(sfull + g), gph);
                 tc_fence_before();
@@ -587,26 +626,27 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 if (++g == NSEG) { g = 0; gph ^= 1; }
                 continue;
             }
-            tmem_ld32(taddr, va);
+            // The whole accumulator goes to registers at once and is handed back to the MMA warp before any of it is
+            // reduced: with only three accumulators for two query blocks, the next tile's MMAs wait for this release.
+            tmem_ld32(taddr, v);
+            tmem_ld32(taddr + 32, v + 32);
+            tmem_ld32(taddr + 64, v + 64);
+            tmem_ld32(taddr + 96, v + 96);
             mbar_wait(smem_u32(sfull + g), gph);
             const uint32_t* doc = seg[g].doc;
             const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
             st.k = 0;
-            tmem_ld_wait32(va);
-            tmem_ld32(taddr + 32, vb);  // in flight while columns 0..31 are reduced
-            process32(va, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-            tmem_ld_wait32(vb);
-            tmem_ld32(taddr + 64, va);
-            process32(vb, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-            tmem_ld_wait32(va);
-            tmem_ld32(taddr + 96, vb);
-            process32(va, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-            tmem_ld_wait32(vb);
-            // every column is in registers: hand the accumulator back before reducing the last 32
+            tmem_ld_wait32(v);
+            tmem_ld_pin32(v + 32);
+            tmem_ld_pin32(v + 64);
+            tmem_ld_pin32(v + 96);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-            process32(vb, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            process32(v, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            process32(v + 32, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            process32(v + 64, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            process32(v + 96, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
             slot += MB;
