@@ -24,6 +24,7 @@
 // segmenter (turns `offsets` into per-tile boundary masks, writes -inf for empty documents), warp 3 idle,
 // warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of query block (w-4)/4).
 #include <cuda.h>
+#include <cuda_bf16.h>
 #include <cstdlib>
 #include <cuda_runtime.h>
 
@@ -39,6 +40,7 @@ constexpr int KB_TILE_BYTES = BN * KB_BYTES;  // 16 KB: one dimension block of o
 constexpr int NSEG = 4;            // depth of the segment-info ring
 constexpr int MAX_STAGES = 14;
 constexpr int MAX_ACC = 4;
+constexpr int MAX_RAW = 4;
 constexpr int TMEM_COLS = 512;
 constexpr int PEND = 16;           // documents parked per epilogue warp before their scores are summed and stored
 constexpr int PEND_PITCH = 33;     // floats per parked document (32 rows + 1: conflict-free column reads)
@@ -52,7 +54,8 @@ struct Params {
     int Q, Nq, Nq_pad;     // queries in this launch
     int row_bytes;         // d * sizeof(element)
     int NKB;               // dimension blocks per row = row_bytes / 128
-    int NS;                // pipeline stages
+    int NS;                // pipeline (operand) stages
+    int NR;                // fp32 inputs: raw fp32 stages that TMA fills and the splitter warps drain
     int NACC;              // accumulators in the TMEM ring
     int acc_col0;          // first TMEM column of the ring (the A operand sits in columns [0, MB*NKB*32))
     uint32_t idesc;
@@ -167,6 +170,23 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
         "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
         "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
         : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+// Two fp32 values -> packed bf16 pairs (first value in the low half): hi = bf16(x) rounded to nearest even,
+// lo = bf16(x - hi); x - hi is exact in fp32, and hi + lo carries 16 to 18 of x's 24 mantissa bits.
+__device__ __forceinline__ void split_pair(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+    const __nv_bfloat162 h = __floats2bfloat162_rn(x0, x1);
+    const float2 hf = __bfloat1622float2(h);
+    const __nv_bfloat162 l = __floats2bfloat162_rn(x0 - hf.x, x1 - hf.y);
+    hi = *reinterpret_cast<const uint32_t*>(&h);
+    lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 __device__ __forceinline__ uint4 ldg_nc16(const void* p) {
     uint4 r;
@@ -348,27 +368,37 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
 }
 
 // KBS: dimension blocks per pipeline stage (2 = a whole 256-byte row block per stage).
-template <int MB, int KBS>
-__global__ void __launch_bounds__(128 + 128 * MB, 1)
+// F32: fp32 inputs (a9).  The tensor pipe has no fp32 MMA, and TF32 alone would break the 1e-5*Nq tolerance, so
+// every fp32 value x is split on the fly into two bf16 values, hi = bf16(x) and lo = bf16(x - hi) (16-18 mantissa
+// bits together), and hi*hi + hi*lo + lo*hi is accumulated in fp32 -- three bf16 MMAs per K step.
+// Four extra "splitter" warps turn each fp32 tile that TMA lands (a raw stage) into a bf16 hi block + lo block (an
+// operand stage, KBS = 2 blocks); the query rows are split once by their epilogue threads.  p.NKB then counts
+// 64-element units (64 fp32 = two 128-byte dimension blocks in, one bf16 hi block + one lo block out).
+template <int MB, int KBS, bool F32>
+__global__ void __launch_bounds__(128 + 128 * MB + (F32 ? 128 : 0), 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    // layout: [stages: NS * KBS*16 KB] [SegInfo x NSEG] [park buffers] [barriers] [misc]
+    // layout: [operand stages: NS * KBS*16 KB] [F32: raw stages: NR * 32 KB] [SegInfo x NSEG] [park buffers] [barriers]
     constexpr uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
+    constexpr uint32_t raw_bytes = 2u * KB_TILE_BYTES;
     constexpr int n_epi_warps = 4 * MB;
     uint8_t* st_ptr = smem;
-    SegInfo* seg = reinterpret_cast<SegInfo*>(st_ptr + (size_t)p.NS * stage_bytes);
+    uint8_t* rw_ptr = st_ptr + (size_t)p.NS * stage_bytes;
+    SegInfo* seg = reinterpret_cast<SegInfo*>(rw_ptr + (F32 ? (size_t)p.NR * raw_bytes : 0));
     float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps][PEND][PEND_PITCH]
     uint32_t* pend_id_all = reinterpret_cast<uint32_t*>(pend_all + n_epi_warps * PEND * PEND_PITCH);  // [warps][PEND]
     uint64_t* bars = reinterpret_cast<uint64_t*>(pend_id_all + n_epi_warps * PEND);
-    uint64_t* full = bars;                       // [NS]   TMA -> MMA
-    uint64_t* empty = full + MAX_STAGES;         // [NS]   MMA -> TMA
-    uint64_t* tdone = empty + MAX_STAGES;        // [4]    MMA -> epilogue: every accumulator of tile t is complete (ring t & 3)
-    uint64_t* tempty = tdone + MAX_ACC;          // [NACC] epilogue -> MMA (4 warps each)
+    uint64_t* full = bars;                       // [NS]   operand stage filled (TMA, or the splitter warps) -> MMA
+    uint64_t* empty = full + MAX_STAGES;         // [NS]   operand stage read by the tensor pipe -> TMA / splitter
+    uint64_t* tfull = empty + MAX_STAGES;        // [4*MB] MMA -> epilogue: accumulator of (tile t, block mb), ring t & 3
+    uint64_t* tempty = tfull + 8;                // [NACC] epilogue -> MMA (4 warps each)
     uint64_t* sfull = tempty + MAX_ACC;          // [NSEG] segmenter -> epilogue
     uint64_t* sempty = sfull + NSEG;             // [NSEG] epilogue -> segmenter
-    uint64_t* aready = sempty + NSEG;            // [1]    query rows are in TMEM
+    uint64_t* rfull = sempty + NSEG;             // [NR]   F32: TMA -> splitter
+    uint64_t* rempty = rfull + MAX_RAW;          // [NR]   F32: splitter -> TMA (4 warps)
+    uint64_t* aready = rempty + MAX_RAW;         // [1]    query rows are in TMEM
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(aready + 1);
     int64_t* range = reinterpret_cast<int64_t*>(aready + 2);  // b_lo, b_hi, t_lo, t_hi
 
@@ -383,8 +413,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0) {
         if (lane == 0) {
-            for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), 1); mbar_init(smem_u32(empty + s), 1); }
-            for (int s = 0; s < MAX_ACC; ++s) { mbar_init(smem_u32(tdone + s), 1); mbar_init(smem_u32(tempty + s), 4); }
+            for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), F32 ? 4 : 1); mbar_init(smem_u32(empty + s), 1); }
+            for (int s = 0; s < 8; ++s) mbar_init(smem_u32(tfull + s), 1);
+            for (int s = 0; s < MAX_ACC; ++s) mbar_init(smem_u32(tempty + s), 4);
+            for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
             for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), n_epi_warps); }
             mbar_init(smem_u32(aready), n_epi_warps);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -414,27 +446,39 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     const uint32_t tmem_base = *tmem_slot;
     const int64_t b_lo = range[0], b_hi = range[1], t_lo = range[2], t_hi = range[3];
     const int64_t ntiles = (t_hi - t_lo + BN - 1) / BN;
-    const int nchunks = p.NKB / KBS;  // pipeline stages consumed per tile
+    const int nchunks = F32 ? p.NKB : p.NKB / KBS;  // operand stages consumed per tile
 
     if (warp == 0) {
         // ===== TMA producer =====
         // The whole warp runs the loop and waits on the barriers; one elected lane issues the copies, so that the
         // compiler emits the uniform-datapath instructions straight-line (no per-active-thread loop).
         const uint64_t pol_docs = policy_evict_first();  // streamed once
-        uint32_t s = 0, ph = 0;  // ring slot and its phase bit
+        uint32_t s = 0, ph = 0;  // ring slot and its phase bit (F32: the raw ring)
+        const uint32_t nring = F32 ? (uint32_t)p.NR : (uint32_t)p.NS;
         for (int64_t t = 0; t < ntiles; ++t) {
             const int tok = (int)(t_lo + t * BN);
             for (int ch = 0; ch < nchunks; ++ch) {
-                mbar_wait(smem_u32(empty + s), ph ^ 1);
-                if (elect_one()) {
-                    mbar_expect_tx(smem_u32(full + s), stage_bytes);
+                if constexpr (F32) {
+                    mbar_wait(smem_u32(rempty + s), ph ^ 1);
+                    if (elect_one()) {
+                        mbar_expect_tx(smem_u32(rfull + s), raw_bytes);
 #pragma unroll
-                    for (int k = 0; k < KBS; ++k)
-                        tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
-                                    smem_u32(full + s), (ch * KBS + k) * p.kb_elems, tok, pol_docs);
+                        for (int k = 0; k < 2; ++k)  // 64 fp32 of every token = two 128-byte dimension blocks
+                            tma_load_2d(smem_u32(rw_ptr + (size_t)s * raw_bytes + k * KB_TILE_BYTES), &map_docs,
+                                        smem_u32(rfull + s), (ch * 2 + k) * p.kb_elems, tok, pol_docs);
+                    }
+                } else {
+                    mbar_wait(smem_u32(empty + s), ph ^ 1);
+                    if (elect_one()) {
+                        mbar_expect_tx(smem_u32(full + s), stage_bytes);
+#pragma unroll
+                        for (int k = 0; k < KBS; ++k)
+                            tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
+                                        smem_u32(full + s), (ch * KBS + k) * p.kb_elems, tok, pol_docs);
+                    }
                 }
                 __syncwarp();
-                if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
+                if (++s == nring) { s = 0; ph ^= 1; }
             }
         }
     } else if (warp == 1) {
@@ -449,7 +493,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const bool skip = (p.debug & 2) != 0;
         const uint32_t nacc = (uint32_t)p.NACC;
         const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
-        const uint32_t a_mb_step = (uint32_t)p.NKB * KB_WORDS;  // TMEM columns of one query block's rows
+        // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
+        const uint32_t a_lo_off = (uint32_t)p.NKB * KB_WORDS;
+        const uint32_t a_mb_step = F32 ? 2 * a_lo_off : a_lo_off;
+        const bool epi_frees_stage = !F32 && nchunks == 1;
         uint32_t s = 0, ph = 0;
         uint32_t slot[MB], tph[MB];
 #pragma unroll
@@ -469,31 +516,41 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     const uint32_t d_tmem = acc0 + slot[mb] * BN;
                     if (elect_one()) {
                         if (!skip) {
+                            if constexpr (F32) {
 #pragma unroll
-                            for (int k = 0; k < KBS; ++k) {
+                                for (int kk = 0; kk < 4; ++kk) {  // four 16-element K steps per 64-element unit
+                                    const uint64_t b_hi = ((uint64_t)DESC_HI << 32) | (b_lo + kk * 2);
+                                    const uint64_t b_lw = ((uint64_t)DESC_HI << 32) | (b_lo + (KB_TILE_BYTES >> 4) + kk * 2);
+                                    const uint32_t a_hi = a_col + mb * a_mb_step + kk * 8;
+                                    tc_mma_ts(d_tmem, a_hi, b_hi, idesc, (ch != 0 || kk != 0) ? 1u : 0u);
+                                    tc_mma_ts(d_tmem, a_hi, b_lw, idesc, 1u);
+                                    tc_mma_ts(d_tmem, a_hi + a_lo_off, b_hi, idesc, 1u);
+                                }
+                            } else {
 #pragma unroll
-                                for (int kk = 0; kk < 4; ++kk) {  // four 32-byte K steps per 128-byte dimension block
-                                    const uint64_t bd =
-                                        ((uint64_t)DESC_HI << 32) | (b_lo + k * (KB_TILE_BYTES >> 4) + kk * 2);
-                                    const uint32_t at = a_col + mb * a_mb_step + k * KB_WORDS + kk * 8;
-                                    if (k == 0 && kk == 0)
-                                        tc_mma_ts(d_tmem, at, bd, idesc, ch != 0);
-                                    else
-                                        tc_mma_ts(d_tmem, at, bd, idesc, 1u);
+                                for (int k = 0; k < KBS; ++k) {
+#pragma unroll
+                                    for (int kk = 0; kk < 4; ++kk) {  // four 32-byte K steps per 128-byte dimension block
+                                        const uint64_t bd =
+                                            ((uint64_t)DESC_HI << 32) | (b_lo + k * (KB_TILE_BYTES >> 4) + kk * 2);
+                                        const uint32_t at = a_col + mb * a_mb_step + k * KB_WORDS + kk * 8;
+                                        if (k == 0 && kk == 0)
+                                            tc_mma_ts(d_tmem, at, bd, idesc, ch != 0);
+                                        else
+                                            tc_mma_ts(d_tmem, at, bd, idesc, 1u);
+                                    }
                                 }
                             }
                         }
-                        if (mb == MB - 1) {
-                            // One commit per tile when a tile is one stage: "tile done" tells the epilogue that the
-                            // accumulators are complete AND that the stage has been read (an epilogue warp hands the
-                            // stage back to the producer).  Each tcgen05.commit costs the tensor pipe a bubble.
-                            if (ch == nchunks - 1) tc_commit(smem_u32(tdone + (uint32_t)(t & 3)));
-                            if (nchunks > 1) tc_commit(smem_u32(empty + s));
-                        }
+                        // accumulator -> epilogue.  When a tile is a single stage, the last block's barrier also tells
+                        // the epilogue that the stage has been read (it hands the stage back to the producer): one
+                        // tcgen05.commit fewer per tile.
+                        if (ch == nchunks - 1) tc_commit(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb));
+                        if (mb == MB - 1 && !epi_frees_stage) tc_commit(smem_u32(empty + s));
                     }
                     __syncwarp();
                 }
-                a_col += KBS * KB_WORDS;
+                a_col += (F32 ? 1 : KBS) * KB_WORDS;
                 if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
             }
 #pragma unroll
@@ -561,6 +618,43 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // documents after the last token of the range can only be empty
         for (int64_t idx = wb + consumed + lane; idx < b_hi; idx += 32)
             for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
+    } else if (F32 && warp >= 4 + n_epi_warps) {
+        // ===== fp32 splitter (F32 only): raw fp32 stage -> bf16 hi block + bf16 lo block of an operand stage =====
+        // Thread r owns token row r of the tile.  Both layouts are the 128-byte swizzle (16-byte piece index XOR
+        // row % 8), so the eight rows a quarter-warp touches in one instruction fall into eight different bank groups.
+        const int r = threadIdx.x - 32 * (4 + n_epi_warps);
+        const uint32_t sw = (uint32_t)(r & 7);
+        uint32_t s = 0, ph = 0, rs = 0, rph = 0;
+        const int64_t nunits = ntiles * nchunks;
+        for (int64_t u = 0; u < nunits; ++u) {
+            mbar_wait(smem_u32(rfull + rs), rph);
+            mbar_wait(smem_u32(empty + s), ph ^ 1);
+            const uint8_t* raw = rw_ptr + (size_t)rs * raw_bytes + r * KB_BYTES;
+            uint8_t* op = st_ptr + (size_t)s * stage_bytes + r * KB_BYTES;
+#pragma unroll
+            for (int oc = 0; oc < 8; ++oc) {  // 8 fp32 (two 16-byte pieces) in -> 8 bf16 hi (one piece) + 8 bf16 lo out
+                const uint8_t* blk = raw + (oc >> 2) * KB_TILE_BYTES;
+                const uint32_t c0 = (uint32_t)(2 * (oc & 3));
+                const float4 x0 = *reinterpret_cast<const float4*>(blk + ((c0 ^ sw) << 4));
+                const float4 x1 = *reinterpret_cast<const float4*>(blk + (((c0 + 1) ^ sw) << 4));
+                uint4 hi, lo;
+                split_pair(x0.x, x0.y, hi.x, lo.x);
+                split_pair(x0.z, x0.w, hi.y, lo.y);
+                split_pair(x1.x, x1.y, hi.z, lo.z);
+                split_pair(x1.z, x1.w, hi.w, lo.w);
+                const uint32_t o = ((uint32_t)oc ^ sw) << 4;
+                *reinterpret_cast<uint4*>(op + o) = hi;
+                *reinterpret_cast<uint4*>(op + KB_TILE_BYTES + o) = lo;
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> tensor-pipe reads
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(smem_u32(full + s));
+                mbar_arrive(smem_u32(rempty + rs));
+            }
+            if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
+            if (++rs == (uint32_t)p.NR) { rs = 0; rph ^= 1; }
+        }
     } else if (warp >= 4) {
         // ===== epilogue: running rowmax, segmented by document; max -> sum =====
         const int ew = warp - 4, mb = ew >> 2, quad = warp & 3;
@@ -568,20 +662,38 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const int q = row / p.Nq_pad, i = row - q * p.Nq_pad;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quad * 32) << 16);
 
-        // a2: the thread's query row -> TMEM columns [mb*NKB*32, +NKB*32), two 16-bit elements per column;
-        // rows no query token owns are zero (finite similarities that never reach a score, A5)
+        // a2: the thread's query row -> TMEM, two 16-bit elements per column: columns [mb*NKB*32, +NKB*32), or for
+        // F32 the bf16 hi halves in [mb*2*NKB*32, +NKB*32) followed by the lo halves.  Rows no query token owns
+        // are zero (finite similarities that never reach a score, A5).
         {
             const bool row_valid = (q < p.Q) && (i < p.Nq);
             const uint8_t* src = static_cast<const uint8_t*>(p.queries) + ((int64_t)q * p.Nq + i) * p.row_bytes;
             for (int kb = 0; kb < p.NKB; ++kb) {
-                uint32_t w[KB_WORDS];
+                if constexpr (F32) {
+#pragma unroll 1
+                    for (int half = 0; half < 2; ++half) {  // 32 fp32 -> 16 columns of hi, 16 columns of lo
+                        uint32_t hi[16], lo[16];
 #pragma unroll
-                for (int j = 0; j < KB_WORDS / 4; ++j) {
-                    uint4 x = make_uint4(0, 0, 0, 0);
-                    if (row_valid) x = ldg_nc16(src + kb * KB_BYTES + j * 16);
-                    w[4 * j] = x.x; w[4 * j + 1] = x.y; w[4 * j + 2] = x.z; w[4 * j + 3] = x.w;
+                        for (int j = 0; j < 8; ++j) {
+                            uint4 x = make_uint4(0, 0, 0, 0);
+                            if (row_valid) x = ldg_nc16(src + kb * 256 + half * 128 + j * 16);
+                            split_pair(__uint_as_float(x.x), __uint_as_float(x.y), hi[2 * j], lo[2 * j]);
+                            split_pair(__uint_as_float(x.z), __uint_as_float(x.w), hi[2 * j + 1], lo[2 * j + 1]);
+                        }
+                        const uint32_t col = (uint32_t)((mb * 2 * p.NKB + kb) * KB_WORDS + half * 16);
+                        tmem_st16(lane_addr + col, hi);
+                        tmem_st16(lane_addr + col + (uint32_t)(p.NKB * KB_WORDS), lo);
+                    }
+                } else {
+                    uint32_t w[KB_WORDS];
+#pragma unroll
+                    for (int j = 0; j < KB_WORDS / 4; ++j) {
+                        uint4 x = make_uint4(0, 0, 0, 0);
+                        if (row_valid) x = ldg_nc16(src + kb * KB_BYTES + j * 16);
+                        w[4 * j] = x.x; w[4 * j + 1] = x.y; w[4 * j + 2] = x.z; w[4 * j + 3] = x.w;
+                    }
+                    tmem_st32(lane_addr + (uint32_t)((mb * p.NKB + kb) * KB_WORDS), w);
                 }
-                tmem_st32(lane_addr + (uint32_t)((mb * p.NKB + kb) * KB_WORDS), w);
             }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
@@ -599,6 +711,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         uint32_t* pend_id = pend_id_all + ew * PEND;
         const bool skip_math = (p.debug & 1) != 0;
         const int64_t B = p.B;
+        const bool frees_stage = !F32 && nchunks == 1 && ew == 4 * (MB - 1);  // see the MMA warp
 
         EpiState st;
         st.m = -INFINITY;  // Alg. 3 line 4
@@ -608,14 +721,13 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t acc0 = lane_addr + (uint32_t)p.acc_col0;
         uint32_t slot = (uint32_t)mb, tph = 0, g = 0, gph = 0, rs = 0;
         for (int64_t t = 0; t < ntiles; ++t) {
-            mbar_wait(smem_u32(tdone + (uint32_t)(t & 3)), (uint32_t)(t >> 2) & 1u);
+            mbar_wait(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb), (uint32_t)(t >> 2) & 1u);
             tc_fence_after();
-            if (nchunks == 1 && ew == 0) {  // the tile's only stage has been read by the tensor pipe: back to the producer
+            if (frees_stage) {  // the tile's only stage has been read by the tensor pipe: back to the producer
                 if (lane == 0) mbar_arrive(smem_u32(empty + rs));
                 if (++rs == (uint32_t)p.NS) rs = 0;
             }
             const uint32_t taddr = acc0 + slot * BN;
-            float v[BN];
             if (p.debug & 4) {  // measurement probe: no TMEM reads at all
                 mbar_wait(smem_u32(sfull + g), gph);
                 tc_fence_before();
@@ -626,27 +738,53 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 if (++g == NSEG) { g = 0; gph ^= 1; }
                 continue;
             }
-            // The whole accumulator goes to registers at once and is handed back to the MMA warp before any of it is
-            // reduced: with only three accumulators for two query blocks, the next tile's MMAs wait for this release.
-            tmem_ld32(taddr, v);
-            tmem_ld32(taddr + 32, v + 32);
-            tmem_ld32(taddr + 64, v + 64);
-            tmem_ld32(taddr + 96, v + 96);
-            mbar_wait(smem_u32(sfull + g), gph);
-            const uint32_t* doc = seg[g].doc;
-            const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
-            st.k = 0;
-            tmem_ld_wait32(v);
-            tmem_ld_pin32(v + 32);
-            tmem_ld_pin32(v + 64);
-            tmem_ld_pin32(v + 96);
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-            process32(v, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-            process32(v + 32, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-            process32(v + 64, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-            process32(v + 96, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            if constexpr (F32) {
+                // 512 threads leave 128 registers each: the accumulator is read in two halves of 64 columns.  A tile
+                // costs the tensor pipe three MMAs per K step here, so the later release is off the critical path.
+                float v[64];
+                tmem_ld32(taddr, v);
+                tmem_ld32(taddr + 32, v + 32);
+                mbar_wait(smem_u32(sfull + g), gph);
+                const uint32_t* doc = seg[g].doc;
+                const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
+                st.k = 0;
+                tmem_ld_wait32(v);
+                tmem_ld_pin32(v + 32);
+                process32(v, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v + 32, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                tmem_ld32(taddr + 64, v);
+                tmem_ld32(taddr + 96, v + 32);
+                tmem_ld_wait32(v);
+                tmem_ld_pin32(v + 32);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
+                process32(v, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v + 32, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            } else {
+                // The whole accumulator goes to registers at once and is handed back to the MMA warp before any of it
+                // is reduced: with three accumulators for two query blocks, the next tile's MMAs wait for this release.
+                float v[BN];
+                tmem_ld32(taddr, v);
+                tmem_ld32(taddr + 32, v + 32);
+                tmem_ld32(taddr + 64, v + 64);
+                tmem_ld32(taddr + 96, v + 96);
+                mbar_wait(smem_u32(sfull + g), gph);
+                const uint32_t* doc = seg[g].doc;
+                const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
+                st.k = 0;
+                tmem_ld_wait32(v);
+                tmem_ld_pin32(v + 32);
+                tmem_ld_pin32(v + 64);
+                tmem_ld_pin32(v + 96);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
+                process32(v, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v + 32, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v + 64, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v + 96, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
             slot += MB;
@@ -714,6 +852,7 @@ int next_pow2(int v) {
 struct Plan {
     Params p;           // per-launch fields (queries, scores, Q) are filled in by the launcher
     int MB, KBS;        // query blocks per launch, dimension blocks per stage
+    bool f32;           // fp32 inputs: split into bf16 pairs on the fly
     int Qg;             // queries per launch
     uint32_t smem_bytes;
 };
@@ -721,23 +860,25 @@ struct Plan {
 uint32_t fixed_smem(int MB) {
     const uint32_t warps = 4u * MB;
     return (uint32_t)sizeof(SegInfo) * NSEG + warps * PEND * (PEND_PITCH + 1) * 4 +
-           8u * (2 * MAX_STAGES + 2 * MAX_ACC + 2 * NSEG + 2) + 4 * 8 + 1024 /* alignment slack */;
+           8u * (2 * MAX_STAGES + 8 + MAX_ACC + 2 * NSEG + 2 * MAX_RAW + 2) + 4 * 8 + 1024 /* alignment slack */;
 }
 
 // Shape -> kernel parameters; false when the tcgen05 path does not cover it.
 bool plan(const DenseArgs& a, Plan& pl) {
     if (a.B <= 0 || a.T <= 0 || a.T >= (1ll << 31) - BN) return false;
-    if (a.dtype == TMS_DTYPE_F32) return false;  // fp32 inputs: plain TF32 would break the 1e-5*Nq tolerance
+    const bool f32 = a.dtype == TMS_DTYPE_F32;
     const int esize = (int)dtype_size(a.dtype);
     const int row_bytes = a.d * esize;
-    if (row_bytes % KB_BYTES != 0) return false;
+    // 16-bit: whole 128-byte dimension blocks; fp32: whole 64-element units (256 bytes)
+    if (row_bytes % (f32 ? 2 * KB_BYTES : KB_BYTES) != 0) return false;
     const int nqp = next_pow2(a.Nq);
     if (nqp > 32) return false;  // a query's rows must sit inside one warp's 32 TMEM lanes
-    const int NKB = row_bytes / KB_BYTES;
-    // TMEM budget: MB*NKB*32 columns of query rows + at least MB accumulators of 128 columns
+    const int NKB = f32 ? a.d / 64 : row_bytes / KB_BYTES;  // fp32: 64-element units
+    // TMEM budget: query rows (fp32: bf16 hi and lo halves) + at least MB accumulators of 128 columns
+    const int a_cols_per_block = (f32 ? 2 : 1) * NKB * KB_WORDS;
     int MB = 2;
-    if (MB * NKB * KB_WORDS + MB * BN > TMEM_COLS) MB = 1;
-    if (MB * NKB * KB_WORDS + MB * BN > TMEM_COLS) return false;  // d too large for a resident query block
+    if (MB * a_cols_per_block + MB * BN > TMEM_COLS) MB = 1;
+    if (MB * a_cols_per_block + MB * BN > TMEM_COLS) return false;  // d too large for a resident query block
     const int per_block = 128 / nqp;  // queries per 128-row block
     if (a.Q <= per_block) MB = 1;
     Params& p = pl.p;
@@ -749,27 +890,33 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.row_bytes = row_bytes;
     p.NKB = NKB;
     p.kb_elems = KB_BYTES / esize;
-    const int a_cols = MB * NKB * KB_WORDS;
-    p.NACC = (TMEM_COLS - a_cols) / BN;
+    p.NACC = (TMEM_COLS - MB * a_cols_per_block) / BN;
     if (p.NACC > MAX_ACC) p.NACC = MAX_ACC;
     p.acc_col0 = TMEM_COLS - p.NACC * BN;
     {
         const char* dbg = getenv("TMS_DEBUG");
         p.debug = dbg ? atoi(dbg) : 0;
     }
-    const uint32_t fmt = a.dtype == TMS_DTYPE_BF16 ? 1u : 0u;
+    const uint32_t fmt = a.dtype == TMS_DTYPE_F16 ? 0u : 1u;  // fp32 inputs are split into bf16 pairs
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     pl.MB = MB;
     pl.Qg = MB * per_block;
-    pl.KBS = (NKB % 2 == 0) ? 2 : 1;
+    pl.f32 = f32;
+    pl.KBS = f32 ? 2 : ((NKB % 2 == 0) ? 2 : 1);
     const uint32_t fixed = fixed_smem(MB);
     const uint32_t stage_bytes = (uint32_t)pl.KBS * KB_TILE_BYTES;
     int ns = (int)((SMEM_LIMIT - fixed) / stage_bytes);
+    p.NR = 0;
+    if (f32) {  // 32 KB raw stages and 32 KB operand stages share the budget
+        p.NR = ns / 2 > MAX_RAW ? MAX_RAW : ns / 2;
+        ns -= p.NR;
+        if (p.NR < 1) return false;
+    }
     p.NS = ns > MAX_STAGES ? MAX_STAGES : ns;
     if (const char* e = getenv("TMS_NS")) { int v = atoi(e); if (v >= 2 && v < p.NS) p.NS = v; }
-    pl.smem_bytes = (uint32_t)p.NS * stage_bytes + fixed;
-    return p.NS >= 2;
+    pl.smem_bytes = (uint32_t)(p.NS + p.NR) * stage_bytes + fixed;
+    return p.NS >= (f32 ? 1 : 2);
 }
 
 }  // namespace
@@ -792,8 +939,9 @@ int launch_dense_tc(const DenseArgs& a) {
         return TMS_ERR_CUDA;
 
     void (*kern)(const CUtensorMap, const Params) = nullptr;
-    if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1> : dense_tc_kernel<1, 2>;
-    else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1> : dense_tc_kernel<2, 2>;
+    if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true> : dense_tc_kernel<2, 2, true>;
+    else if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false> : dense_tc_kernel<1, 2, false>;
+    else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false> : dense_tc_kernel<2, 2, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess)
         return TMS_ERR_CUDA;
     // no more CTAs than 128-token tiles; one CTA per SM
@@ -805,7 +953,7 @@ int launch_dense_tc(const DenseArgs& a) {
         p.Q = a.Q - q0 < pl.Qg ? a.Q - q0 : pl.Qg;
         p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * a.Nq * p.row_bytes;
         p.scores = a.scores + (int64_t)q0 * a.B;
-        kern<<<(unsigned)grid, 128 + 128 * pl.MB, pl.smem_bytes, a.stream>>>(map_docs, p);
+        kern<<<(unsigned)grid, 128 + 128 * pl.MB + (pl.f32 ? 128 : 0), pl.smem_bytes, a.stream>>>(map_docs, p);
         count_launch();
         if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
     }
