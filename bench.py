@@ -50,6 +50,8 @@ WORKLOADS = {
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
 ELEM_BYTES = {"bf16": 2, "fp16": 2, "fp32": 4}
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only when MEASURED_PEAKS.json is absent
+FALLBACK_BF16_TFLOPS = 1590.0
+SMEM_PIPE_PEAK_GBS = 148 * 128 * 1.965  # shared-memory load pipe: SMs x bytes/clk x max SM clock (GHz) = 37,229 GB/s
 
 
 # ---- inputs ----------------------------------------------------------------------------------------------------------
@@ -326,33 +328,52 @@ def main():
     value = world * B / (ms_per_step * 1e-3)
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------------------------
+    # Each step is timed alone (events around one call), so the burst peaks of MEASURED_PEAKS.json apply.
+    from paper_2606_26439_b200 import accounting
+
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(peaks_path):
-        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+        pk = json.load(open(peaks_path))
+        hbm_peak, tc_peak, peak_src = float(pk["hbm_gbs"]), float(pk["bf16_tflops"]), "MEASURED_PEAKS.json (of measured)"
     else:
-        peak, peak_src = FALLBACK_HBM_GBS, "B200_PROFILING.md fallback (of fallback)"
+        hbm_peak, tc_peak, peak_src = FALLBACK_HBM_GBS, FALLBACK_BF16_TFLOPS, "B200_PROFILING.md fallback (of fallback)"
     abytes = algorithmic_bytes(w, T, B)
     kern_ms = float(step_ms.mean())
-    achieved = abytes / (kern_ms * 1e-3) / 1e9
+    kern_s = kern_ms * 1e-3
+    hbm_gbs = abytes / kern_s / 1e9
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(args.workload)
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
-                "kernel_ms_mean": kern_ms, "kernel_ms_min": float(step_ms.min()), "kernel_ms_median": float(np.median(step_ms)),
-                "frac_of_nominal_8000": achieved / 8000.0}
+    common = {"traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
+              "kernel_ms_mean": kern_ms, "kernel_ms_min": float(step_ms.min()),
+              "kernel_ms_median": float(np.median(step_ms)),
+              "hbm": {"achieved_GBps": hbm_gbs, "peak_GBps": hbm_peak, "frac": hbm_gbs / hbm_peak,
+                      "frac_of_nominal_8000": hbm_gbs / 8000.0}}
     if w["kind"] == "dense":
-        from paper_2606_26439_b200 import accounting
-
+        # tensor work: 2*Q*Nq*T*d algorithmic FLOP; fp32 inputs cost three bf16 MMAs per product, so
+        # their tensor peak is a third of the bf16 peak.  The roofline that binds is the one with the larger ideal time.
         fl = accounting.dense_flops(w["Q"], w["Nq"], w["d"], T)
-        roofline["tensor_tflops"] = fl / (kern_ms * 1e-3) / 1e12
+        tc_eff_peak = tc_peak / (3.0 if w["dtype"] == "fp32" else 1.0)
+        tfl = fl / kern_s / 1e12
+        common["tensor"] = {"achieved_TFLOPs": tfl, "peak_TFLOPs": tc_eff_peak, "frac": tfl / tc_eff_peak,
+                            "algorithmic_flops_per_launch": fl}
+        if fl / (tc_eff_peak * 1e12) > abytes / (hbm_peak * 1e9):
+            roofline = {"bound": "tensor", "achieved": tfl, "peak": tc_eff_peak, "unit": "TFLOP/s",
+                        "frac": tfl / tc_eff_peak}
+        else:
+            roofline = {"bound": "hbm", "achieved": hbm_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_gbs / hbm_peak}
+        roofline["tensor_tflops"] = tfl
     else:
-        from paper_2606_26439_b200 import accounting
-
+        # fused PQ: Q*Nq*T*M four-byte shared-memory gathers against M bytes of codes per token -- bound by the
+        # shared-memory load pipe (128 B/clk/SM), not by HBM and not by tensor cores
         lookups = accounting.pq_lookups(w["Q"], w["Nq"], w["M"], T)
-        roofline["lut_gather_GBps"] = lookups * 4 / (kern_ms * 1e-3) / 1e9
-        roofline["note"] = "step = LUT build + relayout + fused lookup kernel; bound by shared-memory gathers (DESIGN.md)"
+        smem_peak = SMEM_PIPE_PEAK_GBS
+        g = lookups * 4 / kern_s / 1e9
+        roofline = {"bound": "alu", "achieved": g, "peak": smem_peak, "unit": "GB/s", "frac": g / smem_peak,
+                    "note": "shared-memory gather bytes/s against 148 SMs x 128 B/clk x 1.965 GHz; step = LUT build + "
+                            "relayout + fused lookup kernel (DESIGN.md 5.4)"}
+    roofline.update(common)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

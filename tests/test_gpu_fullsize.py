@@ -1,0 +1,128 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same entry points, same
+variant selection, same shapes).  The oracle cannot score 500,000 x 8 documents in test time, so each case checks
+
+  * sampled outputs: a seeded sample of documents (plus every planted one) is gathered into a small store and
+    scored one by one by the fp64 oracle; the GPU scores at those indices must agree within the north_star
+    tolerance (1e-5*Nq for fp32, 2e-3*Nq for bf16/fp16 and PQ);
+  * ranking: per query the GPU's top-100 over ALL documents must be the planted documents, position by position
+    (their oracle scores are ~0.126 apart, twice the bf16 tolerance); inside the sample the
+    general rule holds: where GPU and oracle rankings differ, the oracle scores differ by less than the tolerance;
+  * properties that hold at any size: every score finite, |score| <= Nq (unit-norm inputs, bound P4), run-to-run
+    bit-identical.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_26439_b200 import synth, tms
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+TORCH = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
+
+
+def tol(dtype, Nq):
+    return (1e-5 if dtype == torch.float32 else 2e-3) * Nq
+
+
+def gather_docs(store, off, ids):
+    """Sub-store holding documents `ids` (host tensors + offsets) for the oracle."""
+    lens = (off[ids + 1] - off[ids]).astype(np.int64)
+    sub_off = synth.offsets_from_lengths(lens)
+    idx = np.concatenate([np.arange(off[b], off[b + 1]) for b in ids]) if len(ids) else np.zeros(0, np.int64)
+    sub = store[torch.from_numpy(idx).to(store.device)].cpu()
+    return sub, sub_off
+
+
+def ranking_rule(got, ref, atol, k=100):
+    """Positions where the two top-k lists differ must hold documents whose oracle scores are within atol."""
+    for q in range(got.shape[0]):
+        g = np.lexsort((np.arange(got.shape[1]), -got[q]))[:k]
+        o = np.lexsort((np.arange(ref.shape[1]), -ref[q]))[:k]
+        diff = g != o
+        assert np.all(np.abs(ref[q, g[diff]] - ref[q, o[diff]]) < atol)
+
+
+def dense_fullsize(Q, Nq, d, dtype, off, seed, n_sample=1500, planted=True):
+    B, T = len(off) - 1, int(off[-1])
+    q = synth.unit_tokens(Q * Nq, d, dtype, seed=seed + 1, device=DEV).view(Q, Nq, d)
+    D = synth.unit_tokens(T, d, dtype, seed=seed + 2, device=DEV)
+    ids_planted = synth.plant_relevant(q, D, off, seed=seed + 3) if planted else np.zeros((Q, 0), np.int64)
+    off_d = torch.from_numpy(off).to(DEV)
+    got_d = tms.tms_maxsim(q, D, off_d)          # the call bench.py makes (variant "auto")
+    again = tms.tms_maxsim(q, D, off_d)
+    torch.cuda.synchronize()
+    assert torch.equal(got_d, again), "run-to-run bit reproducibility"
+    assert bool(torch.isfinite(got_d).all())
+    assert float(got_d.abs().max()) <= Nq * 1.01, "bound P4: |score| <= Nq for unit-norm tokens"
+
+    rng = np.random.default_rng(seed)
+    sample = np.unique(np.concatenate([rng.choice(B, size=n_sample, replace=False), ids_planted.reshape(-1),
+                                       [0, B - 1]]))
+    sub, sub_off = gather_docs(D, off, sample)
+    ref = oracle.maxsim(q.cpu(), sub, sub_off)
+    got = got_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
+    err = np.abs(got - ref).max()
+    assert err <= tol(dtype, Nq), f"max |dscore| over {len(sample)} sampled documents = {err:.3e}"
+    ranking_rule(got, ref, tol(dtype, Nq))
+    if planted:
+        top = torch.topk(got_d, 100, dim=1).indices.cpu().numpy()
+        assert np.array_equal(top, ids_planted[:, :100]), "top-100 must be the planted documents in order"
+    return err
+
+
+# ---- configs[1]: ColBERT-scale, Q=8, Nq=32, d=128, B=500,000 x Nd=128, all three storage dtypes ---------------------
+
+@pytest.mark.parametrize("dtype", ["bf16", "fp16", "fp32"])
+def test_config1_colbert_scale(dtype):
+    dense_fullsize(8, 32, 128, TORCH[dtype], synth.uniform_offsets(500_000, 128), seed=100)
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("Q", [1, 4])
+def test_config1_fewer_queries(Q):
+    dense_fullsize(Q, 32, 128, torch.bfloat16, synth.uniform_offsets(500_000, 128), seed=110 + Q)
+    torch.cuda.empty_cache()
+
+
+# ---- configs[2]: variable length, lognormal(median 64, sigma 0.5) clipped to [8, 180] --------------------------------
+
+@pytest.mark.parametrize("B", [100_000, 500_000])
+def test_config2_variable_length(B):
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(B, seed=7))
+    dense_fullsize(8, 32, 128, torch.bfloat16, off, seed=200 + B // 1000)
+    torch.cuda.empty_cache()
+
+
+# ---- configs[3]: dimension sweep, Q=4, B=100,000 x Nd=128 ------------------------------------------------------------
+
+@pytest.mark.parametrize("d", [64, 256, 512, 768])
+def test_config3_dimension_sweep(d):
+    dense_fullsize(4, 32, d, torch.bfloat16, synth.uniform_offsets(100_000, 128), seed=300 + d, n_sample=800)
+    torch.cuda.empty_cache()
+
+
+# ---- configs[4]: fused PQ, Q=8, B=1,000,000 x Nd=128, M=16, K=256 ----------------------------------------------------
+
+def test_config4_fused_pq():
+    Q, Nq, d, M, K, B = 8, 32, 128, 16, 256, 1_000_000
+    off = synth.uniform_offsets(B, 128)
+    q = synth.unit_tokens(Q * Nq, d, torch.bfloat16, seed=401, device=DEV).view(Q, Nq, d)
+    C = synth.pq_codebooks(M, K, d // M, seed=402)
+    codes = synth.pq_codes(int(off[-1]), M, seed=403, device=DEV, K=K)
+    off_d = torch.from_numpy(off).to(DEV)
+    lut = tms.tms_pq_build_lut(q, C.to(DEV))
+    got_d = tms.tms_pq_maxsim(lut, codes, off_d)
+    again = tms.tms_pq_maxsim(lut, codes, off_d)
+    torch.cuda.synchronize()
+    assert torch.equal(got_d, again) and bool(torch.isfinite(got_d).all())
+    rng = np.random.default_rng(404)
+    sample = np.unique(np.concatenate([rng.choice(B, size=1500, replace=False), [0, B - 1]]))
+    sub, sub_off = gather_docs(codes, off, sample)
+    ref = oracle.pq_maxsim(q.cpu(), C, sub, sub_off)
+    got = got_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
+    err = np.abs(got - ref).max()
+    assert err <= 2e-3 * Nq, f"max |dscore| = {err:.3e}"
+    ranking_rule(got, ref, 2e-3 * Nq)
+    assert 28.0 < got.mean() < 31.0  # sanity range of configs[4]
