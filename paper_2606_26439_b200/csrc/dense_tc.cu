@@ -43,7 +43,8 @@ constexpr int MAX_ACC = 4;
 constexpr int MAX_RAW = 4;
 constexpr int TMEM_COLS = 512;
 constexpr int PEND = 16;           // documents parked per epilogue warp before their scores are summed and stored
-constexpr int PEND_PITCH = 33;     // floats per parked document (32 rows + 1: conflict-free column reads)
+constexpr int PEND_PITCH = 36;     // floats per parked document: 32 rows, padded so that 16-byte row reads of 8
+                                   // consecutive documents fall into different banks
 constexpr uint32_t SMEM_LIMIT = 232448;  // 227 KB
 
 struct Params {
@@ -238,33 +239,65 @@ __device__ __forceinline__ uint32_t pack_cfg(int Nq, int Nq_pad, int nvalid) {
     return (uint32_t)Nq | ((uint32_t)Nq_pad << 6) | ((uint32_t)nvalid << 12);
 }
 
-// A document's last token has been folded in: row `lane` parks its maximum in slot np of the warp's buffer.
-__device__ __forceinline__ void park(float m, uint32_t k, uint32_t np, float* pend, uint32_t* pend_id,
-                                     const uint32_t* doc, int lane) {
-    pend[np * PEND_PITCH + lane] = m;
-    if (lane == 0) pend_id[np] = doc[k];
+__device__ __forceinline__ void sts_f32(uint32_t addr, float v) {
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ float4 lds_f32x4(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+    return v;
 }
 
-// max -> sum (Eq. 1) for the np parked documents: one lane per (document, query of this warp) adds that query's Nq
-// row maxima in ascending row order and stores the score.  Parked documents are consecutive in the usual case, so
-// the stores of a warp coalesce.
-__device__ __noinline__ void drain(float* pend, const uint32_t* pend_id, uint32_t np, float* out, int64_t B,
-                                   uint32_t cfg, int lane) {
-    const uint32_t Nq = cfg & 63u, Nq_pad = (cfg >> 6) & 63u, nvalid = (cfg >> 12) & 63u;
-    const uint32_t nsub = 32u / Nq_pad;
+// A document's last token has been folded in: row `lane` parks its maximum in slot np of the warp's buffer.
+// pend: shared-window byte address of this warp's park buffer ([PEND][PEND_PITCH] floats, then PEND document ids);
+// doc: shared-window byte address of the current tile's list of ending documents.
+constexpr uint32_t PEND_IDS = PEND * PEND_PITCH * 4;  // byte offset of the ids inside a warp's park buffer
+__device__ __forceinline__ void park(float m, uint32_t k, uint32_t np, uint32_t pend, uint32_t doc, int lane) {
+    sts_f32(pend + (np * PEND_PITCH + lane) * 4, m);
+    if (lane == 0) sts_u32(pend + PEND_IDS + np * 4, lds_u32(doc + k * 4));
+}
+
+// max -> sum (Eq. 1) for the np parked documents.  Rows that no query token owns hold zero query vectors, so their
+// maxima are exactly 0 and every one of the Nq_pad rows of a query can be added (A5).  Parked documents are
+// consecutive in the usual case, so the stores of a warp coalesce.
+//   Nq_pad = 32 (one query per warp): lanes j and j+16 add rows 0..15 / 16..31 of parked document j with four
+//   16-byte loads each, in four interleaved partial sums, and lane j stores the score.
+//   Nq_pad < 32: one lane per (document, query of this warp), rows added in ascending order.
+__device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64_t B, uint32_t cfg, int lane) {
+    const uint32_t Nq_pad = (cfg >> 6) & 63u, nvalid = (cfg >> 12) & 63u;
     __syncwarp();
-    for (uint32_t u = lane; u < np * nsub; u += 32) {
-        const uint32_t slot = u / nsub, sub = u - slot * nsub;
-        if (sub < nvalid) {
-            const float* p = pend + slot * PEND_PITCH + sub * Nq_pad;
-            // all loads first (independent), then four partial sums over rows r = 0,4,8.. / 1,5,.. / 2,6,.. / 3,7,..
-            float x[32];
-#pragma unroll
-            for (int r = 0; r < 32; ++r) x[r] = (uint32_t)r < Nq ? p[r] : 0.f;
-            float a0 = x[0], a1 = x[1], a2 = x[2], a3 = x[3];
-#pragma unroll
-            for (int r = 4; r < 32; r += 4) { a0 += x[r]; a1 += x[r + 1]; a2 += x[r + 2]; a3 += x[r + 3]; }
-            out[(int64_t)sub * B + pend_id[slot]] = (a0 + a1) + (a2 + a3);
+    if (Nq_pad == 32) {
+        const uint32_t j = lane & 15u, h = (uint32_t)lane >> 4;
+        const uint32_t p = pend + (j * PEND_PITCH + h * 16) * 4;
+        const float4 x0 = lds_f32x4(p), x1 = lds_f32x4(p + 16), x2 = lds_f32x4(p + 32), x3 = lds_f32x4(p + 48);
+        const float a0 = (x0.x + x1.x) + (x2.x + x3.x), a1 = (x0.y + x1.y) + (x2.y + x3.y);
+        const float a2 = (x0.z + x1.z) + (x2.z + x3.z), a3 = (x0.w + x1.w) + (x2.w + x3.w);
+        float acc = (a0 + a1) + (a2 + a3);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 16);
+        if (h == 0 && j < np && nvalid) out[lds_u32(pend + PEND_IDS + j * 4)] = acc;
+    } else {
+        const uint32_t nsub = 32u / Nq_pad;
+        for (uint32_t u = lane; u < np * nsub; u += 32) {
+            const uint32_t slot = u / nsub, sub = u - slot * nsub;
+            if (sub < nvalid) {
+                const uint32_t p = pend + (slot * PEND_PITCH + sub * Nq_pad) * 4;
+                float acc = lds_f32(p);
+                for (uint32_t r = 1; r < Nq_pad; ++r) acc += lds_f32(p + r * 4);
+                out[(int64_t)sub * B + lds_u32(pend + PEND_IDS + slot * 4)] = acc;
+            }
         }
     }
     __syncwarp();
@@ -289,14 +322,14 @@ struct EpiState {
 // are folded in order and every finished document is parked.  Out of line: boundary chunks are the minority, and
 // one compact copy keeps the epilogue's hot loop short.  The caller has made sure the buffer has room.
 __device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float x3, float x4, float x5, float x6,
-                                             float x7, uint32_t byte, float m, uint32_t k, uint32_t np, float* pend,
-                                             uint32_t* pend_id, const uint32_t* doc, int lane) {
+                                             float x7, uint32_t byte, float m, uint32_t k, uint32_t np, uint32_t pend,
+                                             uint32_t doc, int lane) {
     const float x[8] = {x0, x1, x2, x3, x4, x5, x6, x7};
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         m = fmaxf(m, x[c]);
         if (byte & (1u << c)) {
-            park(m, k, np, pend, pend_id, doc, lane);
+            park(m, k, np, pend, doc, lane);
             ++k;
             ++np;
             m = -INFINITY;  // Alg. 3 line 4 for the next document
@@ -308,8 +341,7 @@ __device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float
 // 32 accumulator columns (registers v) with boundary word w: bit c set = column c is a document's last token.
 // Words without a boundary (the majority) take sixteen 3-input max instructions, and so does a word whose only
 // boundary is its last column (uniform 128-token documents).  Otherwise the word is walked in 8-column chunks.
-__device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, float* pend, uint32_t* pend_id,
-                                          const uint32_t* doc, float* out, int64_t B, uint32_t cfg, int lane,
+__device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, uint32_t pend, uint32_t doc, float* out, int64_t B, uint32_t cfg, int lane,
                                           bool skip_math) {
     if (skip_math) {  // measurement probe: TMEM loads without the reduction
         s.m = fmaxf(s.m, v[0]);
@@ -321,10 +353,10 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
     }
     if (w == 0x80000000u) {
         if (s.np == PEND) {
-            drain(pend, pend_id, s.np, out, B, cfg, lane);
+            drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
-        park(max33(s.m, v), s.k, s.np, pend, pend_id, doc, lane);
+        park(max33(s.m, v), s.k, s.np, pend, doc, lane);
         ++s.k;
         ++s.np;
         s.m = -INFINITY;
@@ -339,7 +371,7 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
             continue;
         }
         if (s.np + 8 > PEND) {  // room for the up to 8 documents that may end in this chunk
-            drain(pend, pend_id, s.np, out, B, cfg, lane);
+            drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
         if ((byte & (byte - 1)) == 0) {
@@ -353,13 +385,12 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
                 l[c] = left ? x[c] : -INFINITY;
                 r[c] = left ? -INFINITY : x[c];
             }
-            park(max9(s.m, l), s.k, s.np, pend, pend_id, doc, lane);
+            park(max9(s.m, l), s.k, s.np, pend, doc, lane);
             s.m = max9(-INFINITY, r);  // Alg. 3 line 4 for the next document, then its first columns
             ++s.k;
             ++s.np;
         } else {
-            s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.k, s.np, pend, pend_id,
-                                 doc, lane);
+            s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.k, s.np, pend, doc, lane);
             const uint32_t n = __popc(byte);
             s.k += n;
             s.np += n;
@@ -387,9 +418,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint8_t* st_ptr = smem;
     uint8_t* rw_ptr = st_ptr + (size_t)p.NS * stage_bytes;
     SegInfo* seg = reinterpret_cast<SegInfo*>(rw_ptr + (F32 ? (size_t)p.NR * raw_bytes : 0));
-    float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps][PEND][PEND_PITCH]
-    uint32_t* pend_id_all = reinterpret_cast<uint32_t*>(pend_all + n_epi_warps * PEND * PEND_PITCH);  // [warps][PEND]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(pend_id_all + n_epi_warps * PEND);
+    float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps]{[PEND][PEND_PITCH] maxima, [PEND] ids}
+    uint64_t* bars = reinterpret_cast<uint64_t*>(pend_all + n_epi_warps * PEND * (PEND_PITCH + 1));
     uint64_t* full = bars;                       // [NS]   operand stage filled (TMA, or the splitter warps) -> MMA
     uint64_t* empty = full + MAX_STAGES;         // [NS]   operand stage read by the tensor pipe -> TMA / splitter
     uint64_t* tfull = empty + MAX_STAGES;        // [4*MB] MMA -> epilogue: accumulator of (tile t, block mb), ring t & 3
@@ -707,8 +737,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const int nvalid = p.Q - q0 < 0 ? 0 : (p.Q - q0 < nsub ? p.Q - q0 : nsub);
         const uint32_t cfg = pack_cfg(p.Nq, p.Nq_pad, nvalid);
         float* out = p.scores + (int64_t)q0 * p.B + b_lo;
-        float* pend = pend_all + ew * PEND * PEND_PITCH;
-        uint32_t* pend_id = pend_id_all + ew * PEND;
+        const uint32_t pend = smem_u32(pend_all) + (uint32_t)ew * (PEND_IDS + PEND * 4);
         const bool skip_math = (p.debug & 1) != 0;
         const int64_t B = p.B;
         const bool frees_stage = !F32 && nchunks == 1 && ew == 4 * (MB - 1);  // see the MMA warp
@@ -745,13 +774,13 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tmem_ld32(taddr, v);
                 tmem_ld32(taddr + 32, v + 32);
                 mbar_wait(smem_u32(sfull + g), gph);
-                const uint32_t* doc = seg[g].doc;
+                const uint32_t doc = smem_u32(seg[g].doc);
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
                 st.k = 0;
                 tmem_ld_wait32(v);
                 tmem_ld_pin32(v + 32);
-                process32(v, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-                process32(v + 32, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
+                process32(v + 32, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
                 tmem_ld32(taddr + 64, v);
                 tmem_ld32(taddr + 96, v + 32);
                 tmem_ld_wait32(v);
@@ -759,8 +788,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-                process32(v, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-                process32(v + 32, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
+                process32(v + 32, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
             } else {
                 // The whole accumulator goes to registers at once and is handed back to the MMA warp before any of it
                 // is reduced: with three accumulators for two query blocks, the next tile's MMAs wait for this release.
@@ -770,7 +799,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tmem_ld32(taddr + 64, v + 64);
                 tmem_ld32(taddr + 96, v + 96);
                 mbar_wait(smem_u32(sfull + g), gph);
-                const uint32_t* doc = seg[g].doc;
+                const uint32_t doc = smem_u32(seg[g].doc);
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
                 st.k = 0;
                 tmem_ld_wait32(v);
@@ -780,10 +809,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-                process32(v, mask.x, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-                process32(v + 32, mask.y, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-                process32(v + 64, mask.z, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
-                process32(v + 96, mask.w, st, pend, pend_id, doc, out, B, cfg, lane, skip_math);
+                process32(v, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
+                process32(v + 32, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
+                process32(v + 64, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
+                process32(v + 96, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
@@ -791,7 +820,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             if (slot >= nacc) { slot -= nacc; tph ^= 1; }
             if (++g == NSEG) { g = 0; gph ^= 1; }
         }
-        if (st.np) drain(pend, pend_id, st.np, out, B, cfg, lane);
+        if (st.np) drain(pend, st.np, out, B, cfg, lane);
     }
 
     // ---- teardown --------------------------------------------------------------------------------------------
