@@ -51,12 +51,14 @@ static int check_dense(const void* queries, int Q, int Nq, int d, const void* do
 }
 
 static int dense_dispatch(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets,
-                          int64_t B, int64_t T, tms_dtype dtype, float* scores, void* stream, tms_variant variant) {
+                          int64_t B, int64_t T, tms_dtype dtype, float* scores, void* workspace,
+                          size_t workspace_bytes, void* stream, tms_variant variant) {
     int st = check_dense(queries, Q, Nq, d, docs, offsets, B, T, dtype, scores);
     if (st != TMS_OK) return st;
     if (!device_info()) return TMS_ERR_CUDA;
     if (B == 0) return TMS_OK;
-    DenseArgs a{queries, Q, Nq, d, docs, offsets, B, T, dtype, scores, static_cast<cudaStream_t>(stream)};
+    DenseArgs a{queries, Q, Nq, d, docs, offsets, B, T, dtype, scores, static_cast<cudaStream_t>(stream),
+                aligned16(workspace) ? workspace : nullptr, workspace_bytes};
     switch (variant) {
         case TMS_VARIANT_AUTO: return dense_tc_supports(a) ? launch_dense_tc(a) : launch_dense_simt(a);
         case TMS_VARIANT_SIMT: return launch_dense_simt(a);
@@ -102,22 +104,23 @@ extern "C" {
 int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
                int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace, size_t workspace_bytes,
                void* stream) {
-    (void)workspace;
-    (void)workspace_bytes;
-    return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, stream, TMS_VARIANT_AUTO);
+    return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, workspace, workspace_bytes,
+                          stream, TMS_VARIANT_AUTO);
 }
 
 int tms_maxsim_variant(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets,
                        int64_t B, int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace,
                        size_t workspace_bytes, void* stream, tms_variant variant) {
-    (void)workspace;
-    (void)workspace_bytes;
-    return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, stream, variant);
+    return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, workspace, workspace_bytes,
+                          stream, variant);
 }
 
 size_t tms_maxsim_workspace_bytes(int Q, int Nq, int d, int64_t B, tms_dtype dtype) {
-    (void)Q; (void)Nq; (void)d; (void)B; (void)dtype;
-    return 0;  // the dense path needs no scratch: no partial results ever leave the SM
+    (void)d; (void)dtype;
+    // Nq <= 32: no scratch, no partial result ever leaves the SM.  Longer queries are scored as 32-token parts whose
+    // partial scores are added by a second small kernel.
+    if (Q <= 0 || Nq <= 0 || B <= 0) return 0;
+    return dense_tc_workspace_bytes(Q, Nq, B);
 }
 
 int tms_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,

@@ -839,6 +839,17 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     }
 }
 
+// scores[q,b] = sum_j parts[q*nparts + j, b], j ascending (queries longer than 32 tokens)
+__global__ void sum_parts_kernel(const float* __restrict__ parts, float* __restrict__ scores, int Q, int nparts,
+                                 int64_t B) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (int64_t)Q * B) return;
+    const int64_t q = i / B, b = i - q * B;
+    float acc = parts[(q * nparts) * B + b];
+    for (int j = 1; j < nparts; ++j) acc += parts[(q * nparts + j) * B + b];
+    scores[i] = acc;
+}
+
 // ---- host side -----------------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -882,6 +893,7 @@ struct Plan {
     Params p;           // per-launch fields (queries, scores, Q) are filled in by the launcher
     int MB, KBS;        // query blocks per launch, dimension blocks per stage
     bool f32;           // fp32 inputs: split into bf16 pairs on the fly
+    int nparts;         // 32-token parts per query (1 unless Nq > 32)
     int Qg;             // queries per launch
     uint32_t smem_bytes;
 };
@@ -900,8 +912,14 @@ bool plan(const DenseArgs& a, Plan& pl) {
     const int row_bytes = a.d * esize;
     // 16-bit: whole 128-byte dimension blocks; fp32: whole 64-element units (256 bytes)
     if (row_bytes % (f32 ? 2 * KB_BYTES : KB_BYTES) != 0) return false;
-    const int nqp = next_pow2(a.Nq);
-    if (nqp > 32) return false;  // a query's rows must sit inside one warp's 32 TMEM lanes
+    // A query's rows must sit inside one warp's 32 TMEM lanes.  Longer queries (Nq a multiple of 32) are scored as
+    // Nq/32 parts of 32 tokens -- queries[Q,Nq,d] read as [Q*Nq/32, 32, d] -- into a workspace of partial scores that
+    // sum_parts_kernel adds up (Eq. 1's outer sum is associative over query tokens, pin P9).
+    const int nparts = a.Nq > 32 ? a.Nq / 32 : 1;
+    if (a.Nq > 32 && (a.Nq % 32 != 0 || !a.workspace || a.workspace_bytes < dense_tc_workspace_bytes(a.Q, a.Nq, a.B)))
+        return false;
+    const int Nq_part = nparts > 1 ? 32 : a.Nq;
+    const int nqp = next_pow2(Nq_part);
     const int NKB = f32 ? a.d / 64 : row_bytes / KB_BYTES;  // fp32: 64-element units
     // TMEM budget: query rows (fp32: bf16 hi and lo halves) + at least MB accumulators of 128 columns
     const int a_cols_per_block = (f32 ? 2 : 1) * NKB * KB_WORDS;
@@ -909,12 +927,12 @@ bool plan(const DenseArgs& a, Plan& pl) {
     if (MB * a_cols_per_block + MB * BN > TMEM_COLS) MB = 1;
     if (MB * a_cols_per_block + MB * BN > TMEM_COLS) return false;  // d too large for a resident query block
     const int per_block = 128 / nqp;  // queries per 128-row block
-    if (a.Q <= per_block) MB = 1;
+    if (a.Q * nparts <= per_block) MB = 1;
     Params& p = pl.p;
     p.offsets = a.offsets;
     p.B = a.B;
     p.T = a.T;
-    p.Nq = a.Nq;
+    p.Nq = Nq_part;
     p.Nq_pad = nqp;
     p.row_bytes = row_bytes;
     p.NKB = NKB;
@@ -931,6 +949,7 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     pl.MB = MB;
     pl.Qg = MB * per_block;
+    pl.nparts = nparts;
     pl.f32 = f32;
     pl.KBS = f32 ? 2 : ((NKB % 2 == 0) ? 2 : 1);
     const uint32_t fixed = fixed_smem(MB);
@@ -949,6 +968,11 @@ bool plan(const DenseArgs& a, Plan& pl) {
 }
 
 }  // namespace
+
+size_t dense_tc_workspace_bytes(int Q, int Nq, int64_t B) {
+    if (Nq <= 32 || Nq % 32 != 0) return 0;
+    return sizeof(float) * (size_t)Q * (size_t)(Nq / 32) * (size_t)B;
+}
 
 bool dense_tc_supports(const DenseArgs& a) {
     const DeviceInfo* di = device_info();
@@ -977,12 +1001,20 @@ int launch_dense_tc(const DenseArgs& a) {
     int64_t grid = (a.T + BN - 1) / BN;
     if (grid > di->num_sms) grid = di->num_sms;
     // one launch per group of Qg queries (up to 256 query rows): the store is streamed once per group
-    for (int q0 = 0; q0 < a.Q; q0 += pl.Qg) {
+    const int Qeff = a.Q * pl.nparts;  // queries as the kernel sees them (32-token parts of long queries)
+    float* dst = pl.nparts > 1 ? static_cast<float*>(a.workspace) : a.scores;
+    for (int q0 = 0; q0 < Qeff; q0 += pl.Qg) {
         Params p = pl.p;
-        p.Q = a.Q - q0 < pl.Qg ? a.Q - q0 : pl.Qg;
-        p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * a.Nq * p.row_bytes;
-        p.scores = a.scores + (int64_t)q0 * a.B;
+        p.Q = Qeff - q0 < pl.Qg ? Qeff - q0 : pl.Qg;
+        p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * p.Nq * p.row_bytes;
+        p.scores = dst + (int64_t)q0 * a.B;
         kern<<<(unsigned)grid, 128 + 128 * pl.MB + (pl.f32 ? 128 : 0), pl.smem_bytes, a.stream>>>(map_docs, p);
+        count_launch();
+        if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+    }
+    if (pl.nparts > 1) {
+        const int64_t n = (int64_t)a.Q * a.B;
+        sum_parts_kernel<<<(unsigned)((n + 255) / 256), 256, 0, a.stream>>>(dst, a.scores, a.Q, pl.nparts, a.B);
         count_launch();
         if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
     }

@@ -32,6 +32,8 @@ struct DenseArgs {
     tms_dtype dtype;
     float* scores;
     cudaStream_t stream;
+    void* workspace = nullptr;  // device scratch (tms_maxsim_workspace_bytes)
+    size_t workspace_bytes = 0;
 };
 
 // CUDA-core tiled kernel: any dtype / d / Nq / Q (csrc/dense_simt.cu).
@@ -39,6 +41,8 @@ int launch_dense_simt(const DenseArgs& a);
 // TMA + tcgen05 kernel (csrc/dense_tc.cu). supports() says whether the shape is covered.
 bool dense_tc_supports(const DenseArgs& a);
 int launch_dense_tc(const DenseArgs& a);
+// Scratch the tcgen05 path needs for this shape (0 for Nq <= 32).
+size_t dense_tc_workspace_bytes(int Q, int Nq, int64_t B);
 
 // ---- PQ --------------------------------------------------------------------------------------------------------
 struct PqArgs {

@@ -91,7 +91,7 @@ def tms_pq_workspace_bytes(Q, Nq, M, K, B) -> int:
 
 
 def tms_maxsim(queries: torch.Tensor, docs: torch.Tensor, offsets: torch.Tensor, scores: torch.Tensor | None = None,
-               stream=None, variant: str = "auto") -> torch.Tensor:
+               stream=None, variant: str = "auto", workspace: torch.Tensor | None = None) -> torch.Tensor:
     """scores[q,b] = sum_i max_{t in doc b} <queries[q,i], docs[t]>  (include/tms.h: tms_maxsim)."""
     Q, Nq, d = queries.shape
     T = docs.shape[0]
@@ -103,9 +103,15 @@ def tms_maxsim(queries: torch.Tensor, docs: torch.Tensor, offsets: torch.Tensor,
     elif scores.shape != (Q, B) or scores.dtype != torch.float32:
         raise ValueError("scores must be fp32 [Q,B]")
     lib = load()
+    need = int(lib.tms_maxsim_workspace_bytes(Q, Nq, d, B, _DTYPES[queries.dtype]))
+    if workspace is None and need:
+        workspace = torch.empty(need, dtype=torch.uint8, device=queries.device)
+    ws_ptr = _dev(workspace, "workspace") if workspace is not None else None
+    ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
     st = lib.tms_maxsim_variant(_dev(queries, "queries"), Q, Nq, d, _dev(docs, "docs") if T else None,
                                 _dev(offsets, "offsets"), B, T, _DTYPES[queries.dtype],
-                                _dev(scores, "scores") if B else None, None, 0, _stream(stream), VARIANTS[variant])
+                                _dev(scores, "scores") if B else None, ws_ptr, ws_len, _stream(stream),
+                                VARIANTS[variant])
     _check(st, "tms_maxsim")
     return scores
 

@@ -156,6 +156,35 @@ def test_p11_zero_padded_dimensions_tie_the_tiled_variant_to_d128():
         assert np.array_equal(run_dense(qp, Dp, off, "tcgen05"), base)
 
 
+# ---- NEXT-1 shapes: the paper's Nq sweep (Table 10) and Nd sweep (Table 11) -----------------
+
+@pytest.mark.parametrize("Nq", [8, 16, 64, 96])
+def test_query_length_sweep(Nq):
+    off = synth.offsets_from_lengths(np.concatenate([RAGGED, synth.lognormal_lengths(1500, seed=Nq)]))
+    q, D = unit_case(3, Nq, 128, torch.bfloat16, off, seed=40 + Nq)
+    ref = oracle.maxsim(q, D, off)
+    assert_close(run_dense(q, D, off, "tcgen05"), ref, tol(torch.bfloat16, Nq))
+    qi = synth.small_int_tokens(3 * Nq, 128, torch.bfloat16, seed=3).view(3, Nq, 128)
+    Di = synth.small_int_tokens(int(off[-1]), 128, torch.bfloat16, seed=4)
+    assert np.array_equal(run_dense(qi, Di, off, "tcgen05"), oracle.maxsim(qi, Di, off))
+
+
+@pytest.mark.parametrize("Nd", [32, 64, 256, 512])
+def test_document_length_sweep(Nd):
+    off = synth.uniform_offsets(1000, Nd)
+    q, D = unit_case(2, 32, 128, torch.float16, off, seed=60 + Nd)
+    assert_close(run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off), tol(torch.float16, 32))
+
+
+def test_fp32_inputs_on_the_tensor_cores_stay_within_1e5_nq():
+    off = synth.offsets_from_lengths(np.concatenate([RAGGED, synth.lognormal_lengths(6000, seed=9)]))
+    q, D = unit_case(8, 32, 128, torch.float32, off, seed=71)
+    got, ref = run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off)
+    assert_close(got, ref, tol(torch.float32, 32))
+    fin = np.isfinite(ref)
+    assert np.abs(got[fin] - ref[fin]).max() <= 5e-5  # measured ~1e-5: a sixth of the 3.2e-4 tolerance
+
+
 # ---- properties at any size -------------------------------------------------------------------------------------------
 
 def test_run_to_run_bit_reproducible_and_scores_overwritten():
