@@ -790,9 +790,33 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
                 process32(v, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
                 process32(v + 32, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
+            } else if constexpr (MB == 2) {
+                // Two epilogue warps share each scheduler: 32 columns at a time, the next load in flight while the current columns are reduced (a TMEM load of
+                // 32 columns x 32 lanes occupies the warp's TMEM port for about as long as reducing them takes); the
+                // accumulator goes back to the MMA warp as soon as its last column is in registers.
+                float va[32], vb[32];
+                tmem_ld32(taddr, va);
+                mbar_wait(smem_u32(sfull + g), gph);
+                const uint32_t doc = smem_u32(seg[g].doc);
+                const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
+                st.k = 0;
+                tmem_ld_wait32(va);
+                tmem_ld32(taddr + 32, vb);
+                process32(va, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
+                tmem_ld_wait32(vb);
+                tmem_ld32(taddr + 64, va);
+                process32(vb, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
+                tmem_ld_wait32(va);
+                tmem_ld32(taddr + 96, vb);
+                process32(va, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
+                tmem_ld_wait32(vb);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
+                process32(vb, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
             } else {
-                // The whole accumulator goes to registers at once and is handed back to the MMA warp before any of it
-                // is reduced: with three accumulators for two query blocks, the next tile's MMAs wait for this release.
+                // One epilogue warp per scheduler: every extra tcgen05.wait::ld costs more than the overlap gains, so the
+                // whole accumulator is loaded at once and handed back to the MMA warp before any of it is reduced.
                 float v[BN];
                 tmem_ld32(taddr, v);
                 tmem_ld32(taddr + 32, v + 32);
