@@ -45,6 +45,14 @@ WORKLOADS = {
     "c4-d256": dict(kind="dense", Q=4, Nq=32, d=256, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "c4-d512": dict(kind="dense", Q=4, Nq=32, d=512, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "c4-d768": dict(kind="dense", Q=4, Nq=32, d=768, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    # NEXT-1: the paper's query-length and document-length sweeps (Tables 10, 11), Q=1 as in the paper
+    "n1-nq8": dict(kind="dense", Q=1, Nq=8, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    "n1-nq16": dict(kind="dense", Q=1, Nq=16, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    "n1-nq64": dict(kind="dense", Q=1, Nq=64, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    "n1-nd32": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=32, lengths="uniform"),
+    "n1-nd64": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=64, lengths="uniform"),
+    "n1-nd256": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=256, lengths="uniform"),
+    "n1-nd512": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=512, lengths="uniform"),
     "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256),
 }
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
@@ -282,8 +290,11 @@ def main():
         flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     if w["kind"] == "dense":
+        need = tms.tms_maxsim_workspace_bytes(w["Q"], w["Nq"], w["d"], B, TORCH_DTYPES[w["dtype"]])
+        dws = torch.empty(need, dtype=torch.uint8, device=dev) if need else None  # only queries longer than 32 tokens
+
         def step():
-            tms.tms_maxsim(inp["q"], inp["store"], off_d, scores=scores, variant=args.variant)
+            tms.tms_maxsim(inp["q"], inp["store"], off_d, scores=scores, variant=args.variant, workspace=dws)
     else:
         lut = torch.empty((w["Q"], w["Nq"], w["M"], w["K"]), dtype=torch.float32, device=dev)
         ws = torch.empty(max(tms.tms_pq_workspace_bytes(w["Q"], w["Nq"], w["M"], w["K"], B), 16), dtype=torch.uint8,
@@ -342,9 +353,12 @@ def main():
     kern_s = kern_ms * 1e-3
     hbm_gbs = abytes / kern_s / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")  # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(args.workload)
+        for ln in open(tpath).read().splitlines()[1:]:
+            name, _, val = ln.partition(",")
+            if name == args.workload:
+                traffic = int(val)
     common = {"traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
               "kernel_ms_mean": kern_ms, "kernel_ms_min": float(step_ms.min()),
               "kernel_ms_median": float(np.median(step_ms)),
