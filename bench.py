@@ -53,6 +53,9 @@ WORKLOADS = {
     "n1-nd64": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=64, lengths="uniform"),
     "n1-nd256": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=256, lengths="uniform"),
     "n1-nd512": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=512, lengths="uniform"),
+    # NEXT-2: scoring followed by per-query top-100 (the paper's 500K end-to-end case)
+    "c2-topk": dict(kind="dense", Q=8, Nq=32, d=128, dtype="bf16", B=500_000, Nd=128, lengths="uniform", topk=100),
+    "c2-q1-topk": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=500_000, Nd=128, lengths="uniform", topk=100),
     "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256),
 }
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
@@ -293,8 +296,16 @@ def main():
         need = tms.tms_maxsim_workspace_bytes(w["Q"], w["Nq"], w["d"], B, TORCH_DTYPES[w["dtype"]])
         dws = torch.empty(need, dtype=torch.uint8, device=dev) if need else None  # only queries longer than 32 tokens
 
+        k = w.get("topk", 0)
+        if k:
+            tk_v = torch.empty((w["Q"], k), dtype=torch.float32, device=dev)
+            tk_i = torch.empty((w["Q"], k), dtype=torch.int64, device=dev)
+            tk_ws = torch.empty(max(tms.tms_topk_workspace_bytes(w["Q"], B, k), 8), dtype=torch.uint8, device=dev)
+
         def step():
             tms.tms_maxsim(inp["q"], inp["store"], off_d, scores=scores, variant=args.variant, workspace=dws)
+            if k:
+                tms.tms_topk(scores, k, values=tk_v, indices=tk_i, workspace=tk_ws)
     else:
         lut = torch.empty((w["Q"], w["Nq"], w["M"], w["K"]), dtype=torch.float32, device=dev)
         ws = torch.empty(max(tms.tms_pq_workspace_bytes(w["Q"], w["Nq"], w["M"], w["K"], B), 16), dtype=torch.uint8,

@@ -8,6 +8,7 @@
  *                         P:L182-204 Alg. 3).
  *   - tms_pq_build_lut  : product-quantisation distance table, Eq. 8.
  *   - tms_pq_maxsim     : fused lookup + max + sum over uint8 PQ codes, Eq. 9.
+ *   - tms_topk          : per-query top-k over the scores, the step that follows scoring.
  *   - tms_maxsim_host / tms_pq_maxsim_host : the same scoring from HOST buffers, the document store
  *                         streamed through a caller-provided device workspace.
  *
@@ -142,6 +143,20 @@ int tms_pq_maxsim_host(const void* queries, int Q, int Nq, int d, tms_dtype q_dt
 size_t tms_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype dtype, int64_t max_doc_tokens);
 size_t tms_pq_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype q_dtype, int M, int K,
                                               int64_t max_doc_tokens);
+
+/*
+ * Per-query top-k over a score matrix -- the step right after scoring ("followed by torch.topk"):
+ *     for every q: (values[q, r], indices[q, r]), r < k = the k best documents of scores[q, 0..B), ordered by score
+ *     descending, ties by lower document index first; -INFINITY (empty documents) ranks last.
+ * scores   device, fp32 [Q, B] row-major (as written by tms_maxsim / tms_pq_maxsim); not modified; no NaN.
+ * values   device, fp32 [Q, k];   indices  device, int64 [Q, k];   1 <= k <= min(B, 1024);  B <= 2^31.
+ * workspace  device scratch of at least tms_topk_workspace_bytes(Q, B, k) bytes, 8-byte aligned (0 for B <= 4096).
+ * Values are exact copies of the scores; the result is unique and bit-reproducible.
+ */
+int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
+             size_t workspace_bytes, void* stream);
+
+size_t tms_topk_workspace_bytes(int Q, int64_t B, int k);
 
 /* Number of kernels this library has launched in this process since load (all entry points). */
 uint64_t tms_launch_count(void);

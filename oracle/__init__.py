@@ -153,3 +153,15 @@ def pq_maxsim(queries, codebooks, codes, offsets, threads: int = 0, return_threa
 
 def max_threads() -> int:
     return int(_load().oracle_max_threads())
+
+
+def topk(scores, k: int):
+    """Plain definition of per-query top-k (the step after scoring): documents ordered by score descending,
+    ties by lower document index first; returns (values[Q,k] float64, indices[Q,k] int64).
+
+    A stable sort of the negated scores keeps equal scores in index order, which is exactly the tie rule.
+    Pins (tests/test_oracle_pins.py): brute-force selection on tiny inputs, ties, -inf, k = B.
+    """
+    s = np.asarray(scores, dtype=np.float64)
+    order = np.argsort(-s, axis=1, kind="stable")[:, :k]
+    return np.take_along_axis(s, order, axis=1), order.astype(np.int64)

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtms.so")
-SOURCES = ["api.cu", "dense_simt.cu", "dense_tc.cu", "pq.cu", "host_api.cu"]
+SOURCES = ["api.cu", "dense_simt.cu", "dense_tc.cu", "pq.cu", "topk.cu", "host_api.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "--use_fast_math=false"]
 

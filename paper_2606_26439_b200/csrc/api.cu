@@ -153,6 +153,26 @@ size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B) {
     return pq_smem_workspace_bytes(Q, Nq);
 }
 
+int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
+             size_t workspace_bytes, void* stream) {
+    if (Q <= 0 || B <= 0 || k <= 0 || !scores || !values || !indices) return TMS_ERR_INVALID_ARG;
+    if (k > B) return TMS_ERR_INVALID_ARG;
+    if (k > 1024 || B > (1ll << 31) || Q > 65535) return TMS_ERR_UNSUPPORTED;
+    if ((reinterpret_cast<uintptr_t>(scores) & 3u) || (reinterpret_cast<uintptr_t>(values) & 3u) ||
+        (reinterpret_cast<uintptr_t>(indices) & 7u))
+        return TMS_ERR_ALIGNMENT;
+    const size_t need = topk_workspace_bytes(Q, B, k);
+    if (need && (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 7u)))
+        return TMS_ERR_WORKSPACE;
+    if (!device_info()) return TMS_ERR_CUDA;
+    return launch_topk(scores, Q, B, k, values, indices, workspace, static_cast<cudaStream_t>(stream));
+}
+
+size_t tms_topk_workspace_bytes(int Q, int64_t B, int k) {
+    if (Q <= 0 || B <= 0 || k <= 0) return 0;
+    return topk_workspace_bytes(Q, B, k);
+}
+
 uint64_t tms_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char* tms_status_string(int status) {

@@ -61,4 +61,9 @@ bool pq_smem_supports(const PqArgs& a);
 size_t pq_smem_workspace_bytes(int Q, int Nq);
 int launch_pq_smem(const PqArgs& a, void* workspace);
 
+// ---- top-k (csrc/topk.cu) ---------------------------------------------------------------------------------------
+size_t topk_workspace_bytes(int Q, int64_t B, int k);
+int launch_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
+                cudaStream_t stream);
+
 }  // namespace tms

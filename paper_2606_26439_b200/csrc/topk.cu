@@ -1,0 +1,109 @@
+// topk.cu -- per-query top-k over scores[Q, B]: the step right after scoring ("followed by torch.topk ... adding
+// < 0.1 ms").  Order: score descending, ties by lower document index first; -inf
+// (empty documents) sorts last.
+//
+// A score and its document index are packed into one 64-bit key whose unsigned order IS the ranking order:
+// high word = the float's bits mapped monotonically to uint32, low word = ~index.  Level 0 cuts every query's
+// scores into chunks of 4096, sorts each chunk in shared memory (bitonic, descending) and keeps its k best keys;
+// the following levels do the same on the surviving keys until one chunk is left, whose k best are unpacked into
+// values[Q, k] and indices[Q, k].  With k <= 1024 every level shrinks the list at least four-fold.
+#include "tms_internal.h"
+
+namespace tms {
+namespace {
+
+constexpr int CHUNK = 4096;
+constexpr int THREADS = 1024;
+
+__device__ __forceinline__ uint64_t make_key(float score, uint32_t idx) {
+    const uint32_t b = __float_as_uint(score);
+    const uint32_t u = (b & 0x80000000u) ? ~b : (b | 0x80000000u);  // monotone: larger float -> larger u
+    return ((uint64_t)u << 32) | (uint64_t)(~idx);                   // lower index wins a tie
+}
+__device__ __forceinline__ float key_score(uint64_t key) {
+    const uint32_t u = (uint32_t)(key >> 32);
+    return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
+}
+
+// One CTA sorts one chunk of one query's list and emits its `keep` best keys.
+//   scores != nullptr: level 0, the list is scores[q, 0..n)       keys_in == nullptr
+//   else             : the list is keys_in[q, 0..n)
+//   values != nullptr: last level (one chunk): unpack into values / indices instead of keys_out
+__global__ void __launch_bounds__(THREADS)
+topk_level_kernel(const float* __restrict__ scores, const uint64_t* __restrict__ keys_in, int64_t n, int64_t in_pitch,
+                  int keep, uint64_t* __restrict__ keys_out, int64_t out_pitch, float* __restrict__ values,
+                  int64_t* __restrict__ indices, int k) {
+    __shared__ uint64_t key[CHUNK];
+    const int q = blockIdx.y;
+    const int64_t base = (int64_t)blockIdx.x * CHUNK;
+    for (int i = threadIdx.x; i < CHUNK; i += THREADS) {
+        const int64_t j = base + i;
+        uint64_t kk = 0;  // below every real key (a real key's low word is ~index != 0 only for index < 2^32-1;
+                          // its high word is >= 0x007fffff for any non-NaN float)
+        if (j < n) kk = scores ? make_key(scores[(int64_t)q * in_pitch + j], (uint32_t)j) : keys_in[(int64_t)q * in_pitch + j];
+        key[i] = kk;
+    }
+    __syncthreads();
+    // bitonic sort, descending
+    for (int size = 2; size <= CHUNK; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int t = threadIdx.x; t < CHUNK / 2; t += THREADS) {
+                const int lo = 2 * t - (t & (stride - 1));  // index of the pair's first element
+                const int hi = lo + stride;
+                const bool desc = (lo & size) == 0;
+                const uint64_t a = key[lo], b = key[hi];
+                if ((a < b) == desc) { key[lo] = b; key[hi] = a; }
+            }
+            __syncthreads();
+        }
+    }
+    if (values) {
+        for (int i = threadIdx.x; i < k; i += THREADS) {
+            const uint64_t kk = key[i];
+            values[(int64_t)q * k + i] = key_score(kk);
+            indices[(int64_t)q * k + i] = (int64_t)(uint32_t)(~(uint32_t)kk);
+        }
+    } else {
+        for (int i = threadIdx.x; i < keep; i += THREADS)
+            keys_out[(int64_t)q * out_pitch + (int64_t)blockIdx.x * keep + i] = key[i];
+    }
+}
+
+int64_t chunks_of(int64_t n) { return (n + CHUNK - 1) / CHUNK; }
+
+}  // namespace
+
+// two ping-pong key buffers, each sized for level 1's survivors
+size_t topk_workspace_bytes(int Q, int64_t B, int k) {
+    if (B <= CHUNK) return 0;
+    return 2 * sizeof(uint64_t) * (size_t)Q * (size_t)chunks_of(B) * (size_t)k;
+}
+
+int launch_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
+                cudaStream_t stream) {
+    int64_t n = B;
+    const int64_t pitch1 = chunks_of(B) * k;  // keys per query in either buffer (level 1 is the largest)
+    uint64_t* buf[2] = {static_cast<uint64_t*>(workspace), static_cast<uint64_t*>(workspace) + (size_t)Q * pitch1};
+    const float* s_in = scores;
+    const uint64_t* k_in = nullptr;
+    int64_t in_pitch = B;
+    int level = 0;
+    while (true) {
+        const int64_t nch = chunks_of(n);
+        const bool last = nch == 1;
+        dim3 grid((unsigned)nch, (unsigned)Q);
+        topk_level_kernel<<<grid, THREADS, 0, stream>>>(s_in, k_in, n, in_pitch, k, last ? nullptr : buf[level & 1], pitch1,
+                                                        last ? values : nullptr, last ? indices : nullptr, k);
+        count_launch();
+        if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+        if (last) break;
+        s_in = nullptr;
+        k_in = buf[level & 1];
+        in_pitch = pitch1;
+        n = nch * k;
+        ++level;
+    }
+    return TMS_OK;
+}
+
+}  // namespace tms

@@ -34,6 +34,8 @@ SIGNATURES = {
     "tms_pq_maxsim_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i64]),
     "tms_pq_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i, _i, _i64]),
+    "tms_topk": (_i, [_vp, _i, _i64, _i, _vp, _vp, _vp, _sz, _vp]),
+    "tms_topk_workspace_bytes": (_sz, [_i, _i64, _i]),
     "tms_launch_count": (_u64, []),
     "tms_status_string": (ctypes.c_char_p, [_i]),
     "tms_version": (_i, []),
@@ -84,6 +86,10 @@ def tms_version() -> int:
 
 def tms_maxsim_workspace_bytes(Q, Nq, d, B, dtype) -> int:
     return int(load().tms_maxsim_workspace_bytes(Q, Nq, d, B, _DTYPES[dtype]))
+
+
+def tms_topk_workspace_bytes(Q, B, k) -> int:
+    return int(load().tms_topk_workspace_bytes(Q, B, k))
 
 
 def tms_pq_workspace_bytes(Q, Nq, M, K, B) -> int:
@@ -152,6 +158,28 @@ def tms_pq_maxsim(lut: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor,
                                    ws_len, _stream(stream), VARIANTS[variant])
     _check(st, "tms_pq_maxsim")
     return scores
+
+
+def tms_topk(scores: torch.Tensor, k: int, values: torch.Tensor | None = None, indices: torch.Tensor | None = None,
+             workspace: torch.Tensor | None = None, stream=None):
+    """(values[Q,k], indices[Q,k]): per query the k best documents, score descending, ties by lower index first."""
+    Q, B = scores.shape
+    if scores.dtype != torch.float32:
+        raise ValueError("scores must be fp32 [Q,B]")
+    if values is None:
+        values = torch.empty((Q, k), dtype=torch.float32, device=scores.device)
+    if indices is None:
+        indices = torch.empty((Q, k), dtype=torch.int64, device=scores.device)
+    lib = load()
+    need = int(lib.tms_topk_workspace_bytes(Q, B, k))
+    if workspace is None and need:
+        workspace = torch.empty(need, dtype=torch.uint8, device=scores.device)
+    ws_ptr = _dev(workspace, "workspace") if workspace is not None else None
+    ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    st = lib.tms_topk(_dev(scores, "scores"), Q, B, k, _dev(values, "values"), _dev(indices, "indices"), ws_ptr, ws_len,
+                      _stream(stream))
+    _check(st, "tms_topk")
+    return values, indices
 
 
 def _host(t: torch.Tensor, name: str) -> int:

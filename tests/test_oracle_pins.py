@@ -287,3 +287,21 @@ def test_planted_documents_rank_first_in_order():
         gaps = -np.diff(s[qq, top])
         assert gaps.min() > 0.2  # Nq * 0.5 / 49 = 0.33 nominal, far above 2e-3*Nq = 0.064
         assert math.isclose(s[qq, top[0]], 0.95 * Nq, rel_tol=5e-3)
+
+
+# ---- top-k (NEXT-2): the oracle's plain definition against a brute-force selection ------------------------------------
+
+def test_topk_matches_bruteforce_selection_with_ties_and_neg_inf():
+    rng = np.random.default_rng(11)
+    s = rng.integers(-3, 4, size=(3, 40)).astype(np.float64)  # few distinct values: many ties
+    s[0, 5] = s[1, 0] = s[2, 39] = -np.inf
+    for k in (1, 7, 40):
+        vals, idx = oracle.topk(s, k)
+        for q in range(3):
+            left = list(range(40))
+            for r in range(k):  # repeatedly pick the best remaining document: highest score, then lowest index
+                best = max(left, key=lambda b: (s[q, b], -b))
+                left.remove(best)
+                assert idx[q, r] == best and vals[q, r] == s[q, best]
+    vals, idx = oracle.topk(np.array([[1.0, 3.0, 3.0, 2.0]]), 3)
+    assert idx.tolist() == [[1, 2, 3]] and vals.tolist() == [[3.0, 3.0, 2.0]]
