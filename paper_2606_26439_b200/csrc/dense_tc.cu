@@ -61,7 +61,8 @@ struct Params {
     int acc_col0;          // first TMEM column of the ring (the A operand sits in columns [0, MB*NKB*32))
     uint32_t idesc;
     int kb_elems;          // elements per dimension block (64)
-    int debug;             // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs
+    int debug;             // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs, 4 skip TMEM
+                           // reads, 8 write the SM clock seen by each CTA over two scores
 };
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------
@@ -534,12 +535,12 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         for (int64_t t = 0; t < ntiles; ++t) {
             uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
             for (int ch = 0; ch < nchunks; ++ch) {
-                if (!(p.debug & 32)) mbar_wait(smem_u32(full + s), ph);
+                mbar_wait(smem_u32(full + s), ph);
                 tc_fence_after();
                 const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
 #pragma unroll
                 for (int mb = 0; mb < MB; ++mb) {
-                    if (ch == 0 && !(p.debug & 16)) {  // the epilogue has drained this accumulator
+                    if (ch == 0) {  // the epilogue has drained this accumulator
                         mbar_wait(smem_u32(tempty + slot[mb]), tph[mb] ^ 1);
                         tc_fence_after();
                     }
@@ -964,9 +965,9 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.NACC = (TMEM_COLS - MB * a_cols_per_block) / BN;
     if (p.NACC > MAX_ACC) p.NACC = MAX_ACC;
     p.acc_col0 = TMEM_COLS - p.NACC * BN;
-    {
-        const char* dbg = getenv("TMS_DEBUG");
-        p.debug = dbg ? atoi(dbg) : 0;
+    {   // measurement probes, read once per process; 0 in every reported number
+        static const int dbg = [] { const char* e = getenv("TMS_DEBUG"); return e ? atoi(e) & 15 : 0; }();
+        p.debug = dbg;
     }
     const uint32_t fmt = a.dtype == TMS_DTYPE_F16 ? 0u : 1u;  // fp32 inputs are split into bf16 pairs
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
@@ -986,7 +987,6 @@ bool plan(const DenseArgs& a, Plan& pl) {
         if (p.NR < 1) return false;
     }
     p.NS = ns > MAX_STAGES ? MAX_STAGES : ns;
-    if (const char* e = getenv("TMS_NS")) { int v = atoi(e); if (v >= 2 && v < p.NS) p.NS = v; }
     pl.smem_bytes = (uint32_t)(p.NS + p.NR) * stage_bytes + fixed;
     return p.NS >= (f32 ? 1 : 2);
 }
