@@ -371,7 +371,7 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
             s.m = max9(s.m, x);
             continue;
         }
-        if (s.np + 8 > PEND) {  // room for the up to 8 documents that may end in this chunk
+        if (s.np + __popc(byte) > PEND) {  // room for the documents that end in this chunk
             drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
