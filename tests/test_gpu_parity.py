@@ -225,3 +225,40 @@ def test_host_entry_point_streams_chunks():
     small = torch.empty(1 << 16, dtype=torch.uint8, device=DEV)
     with pytest.raises(RuntimeError, match="workspace"):
         tms.tms_maxsim_host(q, D, torch.from_numpy(off), scores, small)
+
+
+# ---- randomised shapes: every path of the tcgen05 kernel against the oracle --------------------------------------------
+
+def _fuzz_lengths(rng, B):
+    kind = rng.integers(0, 5)
+    if kind == 0:   # tiny documents: several boundaries per 8-column chunk, many empties
+        return rng.integers(0, 6, size=B)
+    if kind == 1:   # single-token documents and empties only
+        return rng.integers(0, 2, size=B)
+    if kind == 2:   # the config-2 recipe
+        return synth.lognormal_lengths(B, seed=int(rng.integers(1 << 30)))
+    if kind == 3:   # a few very long documents among short ones
+        lens = rng.integers(1, 40, size=B)
+        lens[rng.integers(0, B, size=max(1, B // 50))] = rng.integers(500, 3000)
+        return lens
+    return np.full(B, int(rng.integers(1, 300)))  # uniform, any length
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_fuzz_shapes_against_the_oracle(seed):
+    rng = np.random.default_rng(1000 + seed)
+    dtype = [torch.bfloat16, torch.float16, torch.float32][seed % 3]
+    d = int(rng.choice([64, 128, 192, 256, 384] if dtype != torch.float32 else [64, 128, 256]))
+    Nq = int(rng.choice([1, 2, 3, 5, 8, 13, 16, 20, 31, 32, 64]))
+    Q = int(rng.integers(1, 21))  # up to 20 queries: several query groups when Q*Nq > 256
+    B = int(rng.integers(1, 1500))
+    lens = _fuzz_lengths(rng, B).astype(np.int64)
+    if lens.sum() == 0:
+        lens[0] = 1
+    off = synth.offsets_from_lengths(lens)
+    q, D = unit_case(Q, Nq, d, dtype, off, seed=seed)
+    ref = oracle.maxsim(q, D, off)
+    assert_close(run_dense(q, D, off, "tcgen05"), ref, tol(dtype, Nq))
+    qi = synth.small_int_tokens(Q * Nq, d, dtype, seed=seed + 1).view(Q, Nq, d)
+    Di = synth.small_int_tokens(int(off[-1]), d, dtype, seed=seed + 2)
+    assert np.array_equal(run_dense(qi, Di, off, "tcgen05"), oracle.maxsim(qi, Di, off))
