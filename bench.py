@@ -389,6 +389,10 @@ def main():
         else:
             roofline = {"bound": "hbm", "achieved": hbm_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_gbs / hbm_peak}
         roofline["tensor_tflops"] = tfl
+        if w["Q"] * w["Nq"] > 128 and w["dtype"] != "fp32":
+            roofline["note"] = ("two query blocks: HBM and tensor ideal times are within 1 % of each other at the burst peaks; the "
+                                "kernel's read stream alone draws 750-950 W of the 1000 W cap, so the tensor pipe runs at a "
+                                "power-capped SM clock of ~1.3 GHz (~1.05 GHz sustained) and binds (DESIGN.md 5.1)")
     else:
         # fused PQ: Q*Nq*T*M four-byte shared-memory gathers against M bytes of codes per token -- bound by the
         # shared-memory load pipe (128 B/clk/SM), not by HBM and not by tensor cores
