@@ -56,6 +56,9 @@ WORKLOADS = {
     # NEXT-2: scoring followed by per-query top-100 (the paper's 500K end-to-end case)
     "c2-topk": dict(kind="dense", Q=8, Nq=32, d=128, dtype="bf16", B=500_000, Nd=128, lengths="uniform", topk=100),
     "c2-q1-topk": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=500_000, Nd=128, lengths="uniform", topk=100),
+    # NEXT-4: the same scores as c5 from the decode-and-contract variant (codebook in shared memory, tensor cores)
+    "c5-decode": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
+                      decode=True),
     "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256),
 }
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
@@ -311,9 +314,13 @@ def main():
         ws = torch.empty(max(tms.tms_pq_workspace_bytes(w["Q"], w["Nq"], w["M"], w["K"], B), 16), dtype=torch.uint8,
                          device=dev)
 
-        def step():
-            tms.tms_pq_build_lut(inp["q"], inp["C"], lut=lut)
-            tms.tms_pq_maxsim(lut, inp["store"], off_d, scores=scores, workspace=ws, variant=args.variant)
+        if w.get("decode"):
+            def step():
+                tms.tms_pq_maxsim_decode(inp["q"], inp["C"], inp["store"], off_d, scores=scores)
+        else:
+            def step():
+                tms.tms_pq_build_lut(inp["q"], inp["C"], lut=lut)
+                tms.tms_pq_maxsim(lut, inp["store"], off_d, scores=scores, workspace=ws, variant=args.variant)
 
     def sync_all():
         torch.cuda.synchronize()
@@ -393,6 +400,14 @@ def main():
             roofline["note"] = ("two query blocks: HBM and tensor ideal times are within 1 % of each other at the burst peaks; the "
                                 "kernel's read stream alone draws 750-950 W of the 1000 W cap, so the tensor pipe runs at a "
                                 "power-capped SM clock of ~1.3 GHz (~1.05 GHz sustained) and binds (DESIGN.md 5.1)")
+    elif w.get("decode"):
+        # decode-and-contract PQ: 2*Q*Nq*T*d FLOP at two bf16 MMAs per product for bf16 queries (hi*hi + hi*lo)
+        fl = accounting.dense_flops(w["Q"], w["Nq"], w["d"], T)
+        tc_eff_peak = tc_peak / 2.0
+        tfl = fl / kern_s / 1e12
+        roofline = {"bound": "tensor", "achieved": tfl, "peak": tc_eff_peak, "unit": "TFLOP/s", "frac": tfl / tc_eff_peak,
+                    "note": "codes decoded in shared memory and contracted on tcgen05; two bf16 MMAs per product "
+                            "(centroids split hi/lo), so the tensor peak is half the bf16 peak (DESIGN.md 10)"}
     else:
         # fused PQ: Q*Nq*T*M four-byte shared-memory gathers against M bytes of codes per token -- bound by the
         # shared-memory load pipe (128 B/clk/SM), not by HBM and not by tensor cores

@@ -8,6 +8,8 @@
  *                         P:L182-204 Alg. 3).
  *   - tms_pq_build_lut  : product-quantisation distance table, Eq. 8.
  *   - tms_pq_maxsim     : fused lookup + max + sum over uint8 PQ codes, Eq. 9.
+ *   - tms_pq_maxsim_decode : the same PQ scores from codes + codebooks, decoded in shared memory and
+ *                         contracted on the tensor cores (no lookup table).
  *   - tms_topk          : per-query top-k over the scores, the step that follows scoring.
  *   - tms_maxsim_host / tms_pq_maxsim_host : the same scoring from HOST buffers, the document store
  *                         streamed through a caller-provided device workspace.
@@ -117,6 +119,21 @@ int tms_pq_maxsim_variant(const float* lut, int Q, int Nq, int M, int K, const u
                           size_t workspace_bytes, void* stream, tms_variant variant);
 
 size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B);
+
+/*
+ * Decode-and-contract PQ scoring: the same value as tms_pq_build_lut + tms_pq_maxsim,
+ *     scores[q*B + b] = sum_{i<Nq}  max_{t in doc b}  <queries[q,i,:], dhat_t>,   dhat_t = concat_m codebooks[m, codes[t,m], :]
+ * (Eq. 9), computed without a lookup table: every tile of 128 tokens is decompressed inside
+ * shared memory from the resident codebook and contracted on the tensor cores; the decompressed vectors never reach
+ * HBM.  Arithmetic: queries and centroids are split into bf16 hi + lo parts (hi*hi + hi*lo + lo*hi, fp32
+ * accumulate), i.e. about 16 mantissa bits per factor -- the result agrees with tms_pq_maxsim to ~1e-5.
+ * Supported: d = 128, M = 16, K = 256 (8-dimensional sub-vectors); any Q; Nq <= 32 or a multiple of 32 (then
+ * `workspace` as for tms_maxsim: tms_maxsim_workspace_bytes(Q, Nq, d, B, q_dtype)); otherwise TMS_ERR_UNSUPPORTED.
+ * queries device [Q, Nq, d] `q_dtype`;  codebooks device fp32 [M, K, d/M];  codes device uint8 [total_tokens, M].
+ */
+int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                         int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
+                         float* scores, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * Host-buffer entry points: identical results, but `queries`, `docs` / `codes`, `offsets`, `codebooks` and

@@ -153,6 +153,26 @@ size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B) {
     return pq_smem_workspace_bytes(Q, Nq);
 }
 
+int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                         int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
+                         float* scores, void* workspace, size_t workspace_bytes, void* stream) {
+    if (Q <= 0 || Nq <= 0 || d <= 0 || M <= 0 || K <= 0 || B < 0 || total_tokens < 0) return TMS_ERR_INVALID_ARG;
+    if (q_dtype != TMS_DTYPE_F32 && q_dtype != TMS_DTYPE_F16 && q_dtype != TMS_DTYPE_BF16) return TMS_ERR_INVALID_ARG;
+    if (!queries || !codebooks || !offsets || (B > 0 && !scores) || (total_tokens > 0 && !codes))
+        return TMS_ERR_INVALID_ARG;
+    if (d != 128 || M != 16 || K != 256) return TMS_ERR_UNSUPPORTED;  // the shape of BASELINE.json configs[4]
+    if (!aligned16(queries) || !aligned16(codebooks) || !aligned16(codes) || (reinterpret_cast<uintptr_t>(offsets) & 7u) ||
+        (reinterpret_cast<uintptr_t>(scores) & 3u))
+        return TMS_ERR_ALIGNMENT;
+    if (!device_info()) return TMS_ERR_CUDA;
+    if (B == 0) return TMS_OK;
+    DenseArgs a{queries, Q, Nq, d, nullptr, offsets, B, total_tokens, q_dtype, scores, static_cast<cudaStream_t>(stream),
+                aligned16(workspace) ? workspace : nullptr, workspace_bytes};
+    a.codes = codes;
+    a.codebooks = codebooks;
+    return dense_tc_supports(a) ? launch_dense_tc(a) : TMS_ERR_UNSUPPORTED;
+}
+
 int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
              size_t workspace_bytes, void* stream) {
     if (Q <= 0 || B <= 0 || k <= 0 || !scores || !values || !indices) return TMS_ERR_INVALID_ARG;

@@ -25,6 +25,7 @@
 // warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of query block (w-4)/4).
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cstdlib>
 #include <cuda_runtime.h>
 
@@ -61,6 +62,11 @@ struct Params {
     int acc_col0;          // first TMEM column of the ring (the A operand sits in columns [0, MB*NKB*32))
     uint32_t idesc;
     int kb_elems;          // elements per dimension block (64)
+    // PQD (decode-and-contract PQ variant): the store is uint8 codes[T,16] + fp32 codebooks[16,256,8]
+    const uint8_t* codes;
+    const float* codebooks;
+    int q_fmt;             // element type of the query rows: 0 fp32, 1 fp16, 2 bf16 (fp32-split paths only)
+    int skip_alo;          // the queries' lo halves are all zero (bf16 queries): leave out the a_lo * b_hi MMAs
     int debug;             // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs, 4 skip TMEM
                            // reads, 8 write the SM clock seen by each CTA over two scores
 };
@@ -97,6 +103,12 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         " [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(dst),
         "l"(map), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
         : "memory");
+}
+// 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (size and addresses multiples of 16)
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
 }
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
@@ -406,7 +418,12 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
 // Four extra "splitter" warps turn each fp32 tile that TMA lands (a raw stage) into a bf16 hi block + lo block (an
 // operand stage, KBS = 2 blocks); the query rows are split once by their epilogue threads.  p.NKB then counts
 // 64-element units (64 fp32 = two 128-byte dimension blocks in, one bf16 hi block + one lo block out).
-template <int MB, int KBS, bool F32>
+// PQD (with F32): the document tile is not loaded but DECODED: TMA brings 128 tokens x 16 code bytes, and the four
+// splitter warps gather every token's 16 centroid slices (8 fp32 each) from the codebook, resident in shared memory,
+// split them into bf16 hi/lo and write the same operand stages as the fp32 path.  The decompressed vectors exist only
+// as MMA operands in shared memory, never in HBM (P:L244-249 names decompress-then-score as the costly baseline
+// because of its HBM round trip; on-chip it costs 16 bytes of HBM per token and no lookup per query row).
+template <int MB, int KBS, bool F32, bool PQD>
 __global__ void __launch_bounds__(128 + 128 * MB + (F32 ? 128 : 0), 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -414,11 +431,13 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     // layout: [operand stages: NS * KBS*16 KB] [F32: raw stages: NR * 32 KB] [SegInfo x NSEG] [park buffers] [barriers]
     constexpr uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
-    constexpr uint32_t raw_bytes = 2u * KB_TILE_BYTES;
+    constexpr uint32_t raw_bytes = PQD ? BN * 16u : 2u * KB_TILE_BYTES;  // PQD: 16 code bytes per token
+    constexpr uint32_t cb_bytes = PQD ? 16u * 256u * 8u * 4u : 0u;        // PQD: the codebook, [16][256][8] fp32
     constexpr int n_epi_warps = 4 * MB;
     uint8_t* st_ptr = smem;
     uint8_t* rw_ptr = st_ptr + (size_t)p.NS * stage_bytes;
-    SegInfo* seg = reinterpret_cast<SegInfo*>(rw_ptr + (F32 ? (size_t)p.NR * raw_bytes : 0));
+    uint8_t* cb_ptr = rw_ptr + (F32 ? (size_t)p.NR * raw_bytes : 0);
+    SegInfo* seg = reinterpret_cast<SegInfo*>(cb_ptr + cb_bytes);
     float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps]{[PEND][PEND_PITCH] maxima, [PEND] ids}
     uint64_t* bars = reinterpret_cast<uint64_t*>(pend_all + n_epi_warps * PEND * (PEND_PITCH + 1));
     uint64_t* full = bars;                       // [NS]   operand stage filled (TMA, or the splitter warps) -> MMA
@@ -429,7 +448,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint64_t* sempty = sfull + NSEG;             // [NSEG] epilogue -> segmenter
     uint64_t* rfull = sempty + NSEG;             // [NR]   F32: TMA -> splitter
     uint64_t* rempty = rfull + MAX_RAW;          // [NR]   F32: splitter -> TMA (4 warps)
-    uint64_t* aready = rempty + MAX_RAW;         // [1]    query rows are in TMEM
+    uint64_t* cbfull = rempty + MAX_RAW;         // [1]    PQD: the codebook has landed in shared memory
+    uint64_t* aready = cbfull + 1;               // [1]    query rows are in TMEM
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(aready + 1);
     int64_t* range = reinterpret_cast<int64_t*>(aready + 2);  // b_lo, b_hi, t_lo, t_hi
 
@@ -450,8 +470,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
             for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), n_epi_warps); }
             mbar_init(smem_u32(aready), n_epi_warps);
+            mbar_init(smem_u32(cbfull), 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
+            if (!PQD) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
         }
         // work partition (a3): documents [b_lo, b_hi) whose first tokens lie in [c*T/G, (c+1)*T/G)
         const int64_t G = gridDim.x, c = blockIdx.x;
@@ -486,7 +507,29 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint64_t pol_docs = policy_evict_first();  // streamed once
         uint32_t s = 0, ph = 0;  // ring slot and its phase bit (F32: the raw ring)
         const uint32_t nring = F32 ? (uint32_t)p.NR : (uint32_t)p.NS;
-        for (int64_t t = 0; t < ntiles; ++t) {
+        if constexpr (PQD) {
+            if (elect_one()) {  // the codebook, once: 128 KB in four bulk copies
+                mbar_expect_tx(smem_u32(cbfull), cb_bytes);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    bulk_load(smem_u32(cb_ptr + k * (cb_bytes / 4)),
+                              reinterpret_cast<const uint8_t*>(p.codebooks) + k * (cb_bytes / 4), cb_bytes / 4,
+                              smem_u32(cbfull));
+            }
+            __syncwarp();
+        }
+        for (int64_t t = 0; PQD && t < ntiles; ++t) {  // one raw stage per tile: the tile's code rows
+            const int64_t tok = t_lo + t * BN;
+            const uint32_t bytes = (uint32_t)((p.T - tok < BN ? p.T - tok : BN) * 16);
+            mbar_wait(smem_u32(rempty + s), ph ^ 1);
+            if (elect_one()) {
+                mbar_expect_tx(smem_u32(rfull + s), bytes);
+                bulk_load(smem_u32(rw_ptr + (size_t)s * raw_bytes), p.codes + tok * 16, bytes, smem_u32(rfull + s));
+            }
+            __syncwarp();
+            if (++s == nring) { s = 0; ph ^= 1; }
+        }
+        for (int64_t t = 0; !PQD && t < ntiles; ++t) {
             const int tok = (int)(t_lo + t * BN);
             for (int ch = 0; ch < nchunks; ++ch) {
                 if constexpr (F32) {
@@ -521,7 +564,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         tc_fence_after();
         const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
         const uint32_t idesc = p.idesc;
-        const bool skip = (p.debug & 2) != 0;
+        const bool skip = (p.debug & 2) != 0, skip_alo = p.skip_alo != 0;
         const uint32_t nacc = (uint32_t)p.NACC;
         const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
         // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
@@ -555,7 +598,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                                     const uint32_t a_hi = a_col + mb * a_mb_step + kk * 8;
                                     tc_mma_ts(d_tmem, a_hi, b_hi, idesc, (ch != 0 || kk != 0) ? 1u : 0u);
                                     tc_mma_ts(d_tmem, a_hi, b_lw, idesc, 1u);
-                                    tc_mma_ts(d_tmem, a_hi + a_lo_off, b_hi, idesc, 1u);
+                                    if (!skip_alo) tc_mma_ts(d_tmem, a_hi + a_lo_off, b_hi, idesc, 1u);
                                 }
                             } else {
 #pragma unroll
@@ -657,7 +700,43 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t sw = (uint32_t)(r & 7);
         uint32_t s = 0, ph = 0, rs = 0, rph = 0;
         const int64_t nunits = ntiles * nchunks;
-        for (int64_t u = 0; u < nunits; ++u) {
+        if constexpr (PQD) {
+            // decode: token row r's 16 codes -> per 64-dimension unit, eight centroid slices of 8 fp32 from the codebook
+            mbar_wait(smem_u32(cbfull), 0);
+            for (int64_t t = 0; t < ntiles; ++t) {
+                mbar_wait(smem_u32(rfull + rs), rph);
+                const uint4 cw = *reinterpret_cast<const uint4*>(rw_ptr + (size_t)rs * raw_bytes + r * 16);
+                const uint32_t cword[4] = {cw.x, cw.y, cw.z, cw.w};
+                for (int ch = 0; ch < nchunks; ++ch) {
+                    mbar_wait(smem_u32(empty + s), ph ^ 1);
+                    uint8_t* op = st_ptr + (size_t)s * stage_bytes + r * KB_BYTES;
+#pragma unroll
+                    for (int oc = 0; oc < 8; ++oc) {  // sub-quantiser m = 8*ch + oc fills 16-byte piece oc of the unit
+                        const uint32_t wsel = ch == 0 ? (oc < 4 ? cword[0] : cword[1]) : (oc < 4 ? cword[2] : cword[3]);
+                        const uint32_t code = (wsel >> (8 * (oc & 3))) & 0xffu;
+                        const uint8_t* e = cb_ptr + ((size_t)((8 * ch + oc) * 256 + code) << 5);
+                        const float4 x0 = *reinterpret_cast<const float4*>(e);
+                        const float4 x1 = *reinterpret_cast<const float4*>(e + 16);
+                        uint4 hi, lo;
+                        split_pair(x0.x, x0.y, hi.x, lo.x);
+                        split_pair(x0.z, x0.w, hi.y, lo.y);
+                        split_pair(x1.x, x1.y, hi.z, lo.z);
+                        split_pair(x1.z, x1.w, hi.w, lo.w);
+                        const uint32_t o = ((uint32_t)oc ^ sw) << 4;
+                        *reinterpret_cast<uint4*>(op + o) = hi;
+                        *reinterpret_cast<uint4*>(op + KB_TILE_BYTES + o) = lo;
+                    }
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(smem_u32(full + s));
+                    if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(rempty + rs));
+                if (++rs == (uint32_t)p.NR) { rs = 0; rph ^= 1; }
+            }
+        }
+        for (int64_t u = 0; !PQD && u < nunits; ++u) {
             mbar_wait(smem_u32(rfull + rs), rph);
             mbar_wait(smem_u32(empty + s), ph ^ 1);
             const uint8_t* raw = rw_ptr + (size_t)rs * raw_bytes + r * KB_BYTES;
@@ -704,12 +783,34 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
 #pragma unroll 1
                     for (int half = 0; half < 2; ++half) {  // 32 fp32 -> 16 columns of hi, 16 columns of lo
                         uint32_t hi[16], lo[16];
+                        if (p.q_fmt == 0) {  // fp32 query rows
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            uint4 x = make_uint4(0, 0, 0, 0);
-                            if (row_valid) x = ldg_nc16(src + kb * 256 + half * 128 + j * 16);
-                            split_pair(__uint_as_float(x.x), __uint_as_float(x.y), hi[2 * j], lo[2 * j]);
-                            split_pair(__uint_as_float(x.z), __uint_as_float(x.w), hi[2 * j + 1], lo[2 * j + 1]);
+                            for (int j = 0; j < 8; ++j) {
+                                uint4 x = make_uint4(0, 0, 0, 0);
+                                if (row_valid) x = ldg_nc16(src + kb * 256 + half * 128 + j * 16);
+                                split_pair(__uint_as_float(x.x), __uint_as_float(x.y), hi[2 * j], lo[2 * j]);
+                                split_pair(__uint_as_float(x.z), __uint_as_float(x.w), hi[2 * j + 1], lo[2 * j + 1]);
+                            }
+                        } else {             // 16-bit query rows (PQD): widened exactly to fp32 first
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                uint4 x = make_uint4(0, 0, 0, 0);
+                                if (row_valid) x = ldg_nc16(src + kb * 128 + half * 64 + j * 16);
+                                const uint32_t w4[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    float f0, f1;
+                                    if (p.q_fmt == 2) {  // bf16: the upper half of an fp32
+                                        f0 = __uint_as_float(w4[e] << 16);
+                                        f1 = __uint_as_float(w4[e] & 0xffff0000u);
+                                    } else {
+                                        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w4[e]));
+                                        f0 = f.x;
+                                        f1 = f.y;
+                                    }
+                                    split_pair(f0, f1, hi[4 * j + e], lo[4 * j + e]);
+                                }
+                            }
                         }
                         const uint32_t col = (uint32_t)((mb * 2 * p.NKB + kb) * KB_WORDS + half * 16);
                         tmem_st16(lane_addr + col, hi);
@@ -918,6 +1019,7 @@ struct Plan {
     Params p;           // per-launch fields (queries, scores, Q) are filled in by the launcher
     int MB, KBS;        // query blocks per launch, dimension blocks per stage
     bool f32;           // fp32 inputs: split into bf16 pairs on the fly
+    bool pqd;           // decode-and-contract PQ variant
     int nparts;         // 32-token parts per query (1 unless Nq > 32)
     int Qg;             // queries per launch
     uint32_t smem_bytes;
@@ -932,11 +1034,13 @@ uint32_t fixed_smem(int MB) {
 // Shape -> kernel parameters; false when the tcgen05 path does not cover it.
 bool plan(const DenseArgs& a, Plan& pl) {
     if (a.B <= 0 || a.T <= 0 || a.T >= (1ll << 31) - BN) return false;
-    const bool f32 = a.dtype == TMS_DTYPE_F32;
+    const bool pqd = a.codes != nullptr;  // decode-and-contract PQ: fp32-split machinery, 16-bit or fp32 queries
+    if (pqd && (a.d != 128 || !a.codebooks)) return false;
+    const bool f32 = pqd || a.dtype == TMS_DTYPE_F32;
     const int esize = (int)dtype_size(a.dtype);
-    const int row_bytes = a.d * esize;
+    const int row_bytes = a.d * esize;  // of a query row; also of a document row unless pqd
     // 16-bit: whole 128-byte dimension blocks; fp32: whole 64-element units (256 bytes)
-    if (row_bytes % (f32 ? 2 * KB_BYTES : KB_BYTES) != 0) return false;
+    if (!pqd && row_bytes % (f32 ? 2 * KB_BYTES : KB_BYTES) != 0) return false;
     // A query's rows must sit inside one warp's 32 TMEM lanes.  Longer queries (Nq a multiple of 32) are scored as
     // Nq/32 parts of 32 tokens -- queries[Q,Nq,d] read as [Q*Nq/32, 32, d] -- into a workspace of partial scores that
     // sum_parts_kernel adds up (Eq. 1's outer sum is associative over query tokens, pin P9).
@@ -962,6 +1066,10 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.row_bytes = row_bytes;
     p.NKB = NKB;
     p.kb_elems = KB_BYTES / esize;
+    p.codes = a.codes;
+    p.codebooks = a.codebooks;
+    p.q_fmt = (int)a.dtype;  // tms_dtype: 0 fp32, 1 fp16, 2 bf16
+    p.skip_alo = pqd && a.dtype == TMS_DTYPE_BF16;  // bf16 queries split into (x, 0)
     p.NACC = (TMEM_COLS - MB * a_cols_per_block) / BN;
     if (p.NACC > MAX_ACC) p.NACC = MAX_ACC;
     p.acc_col0 = TMEM_COLS - p.NACC * BN;
@@ -969,18 +1077,28 @@ bool plan(const DenseArgs& a, Plan& pl) {
         static const int dbg = [] { const char* e = getenv("TMS_DEBUG"); return e ? atoi(e) & 15 : 0; }();
         p.debug = dbg;
     }
-    const uint32_t fmt = a.dtype == TMS_DTYPE_F16 ? 0u : 1u;  // fp32 inputs are split into bf16 pairs
+    const uint32_t fmt = (!f32 && a.dtype == TMS_DTYPE_F16) ? 0u : 1u;  // the split paths feed bf16 pairs
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     pl.MB = MB;
     pl.Qg = MB * per_block;
     pl.nparts = nparts;
     pl.f32 = f32;
+    pl.pqd = pqd;
     pl.KBS = f32 ? 2 : ((NKB % 2 == 0) ? 2 : 1);
     const uint32_t fixed = fixed_smem(MB);
     const uint32_t stage_bytes = (uint32_t)pl.KBS * KB_TILE_BYTES;
     int ns = (int)((SMEM_LIMIT - fixed) / stage_bytes);
     p.NR = 0;
+    if (pqd) {  // 128 KB codebook + four 2 KB code stages, the rest for 32 KB operand stages
+        const uint32_t cb = 16u * 256u * 8u * 4u, raw = MAX_RAW * BN * 16u;
+        if (fixed + cb + raw + stage_bytes > SMEM_LIMIT) return false;
+        p.NR = MAX_RAW;
+        ns = (int)((SMEM_LIMIT - fixed - cb - raw) / stage_bytes);
+        p.NS = ns > MAX_STAGES ? MAX_STAGES : ns;
+        pl.smem_bytes = (uint32_t)p.NS * stage_bytes + raw + cb + fixed;
+        return p.NS >= 1;
+    }
     if (f32) {  // 32 KB raw stages and 32 KB operand stages share the budget
         p.NR = ns / 2 > MAX_RAW ? MAX_RAW : ns / 2;
         ns -= p.NR;
@@ -1011,14 +1129,16 @@ int launch_dense_tc(const DenseArgs& a) {
     Plan pl;
     if (di->cc_major != 10 || !plan(a, pl) || pl.smem_bytes > (uint32_t)di->max_smem_optin) return TMS_ERR_UNSUPPORTED;
 
-    CUtensorMap map_docs;
-    if (!make_map_2d(&map_docs, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d, (uint32_t)pl.p.kb_elems, BN))
+    CUtensorMap map_docs = {};  // unused by the PQ decode variant
+    if (!pl.pqd &&
+        !make_map_2d(&map_docs, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d, (uint32_t)pl.p.kb_elems, BN))
         return TMS_ERR_CUDA;
 
     void (*kern)(const CUtensorMap, const Params) = nullptr;
-    if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true> : dense_tc_kernel<2, 2, true>;
-    else if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false> : dense_tc_kernel<1, 2, false>;
-    else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false> : dense_tc_kernel<2, 2, false>;
+    if (pl.pqd) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, true> : dense_tc_kernel<2, 2, true, true>;
+    else if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, false> : dense_tc_kernel<2, 2, true, false>;
+    else if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false> : dense_tc_kernel<1, 2, false, false>;
+    else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false> : dense_tc_kernel<2, 2, false, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess)
         return TMS_ERR_CUDA;
     // no more CTAs than 128-token tiles; one CTA per SM

@@ -34,6 +34,10 @@ struct DenseArgs {
     cudaStream_t stream;
     void* workspace = nullptr;  // device scratch (tms_maxsim_workspace_bytes)
     size_t workspace_bytes = 0;
+    // decode-and-contract PQ variant: `docs` is unused, the store is codes[T,16] + codebooks[16,256,8]; `dtype` is the
+    // queries' dtype and d = 128
+    const uint8_t* codes = nullptr;
+    const float* codebooks = nullptr;
 };
 
 // CUDA-core tiled kernel: any dtype / d / Nq / Q (csrc/dense_simt.cu).

@@ -30,6 +30,7 @@ SIGNATURES = {
     "tms_pq_maxsim": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
     "tms_pq_workspace_bytes": (_sz, [_i, _i, _i, _i, _i64]),
+    "tms_pq_maxsim_decode": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_maxsim_host": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i64]),
@@ -157,6 +158,32 @@ def tms_pq_maxsim(lut: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor,
                                    _dev(offsets, "offsets"), B, T, _dev(scores, "scores") if B else None, ws_ptr,
                                    ws_len, _stream(stream), VARIANTS[variant])
     _check(st, "tms_pq_maxsim")
+    return scores
+
+
+def tms_pq_maxsim_decode(queries: torch.Tensor, codebooks: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor,
+                         scores: torch.Tensor | None = None, workspace: torch.Tensor | None = None,
+                         stream=None) -> torch.Tensor:
+    """Same value as tms_pq_build_lut + tms_pq_maxsim, decoded tile by tile in shared memory and contracted on the
+    tensor cores (include/tms.h: tms_pq_maxsim_decode)."""
+    Q, Nq, d = queries.shape
+    M, K, dsub = codebooks.shape
+    T, B = codes.shape[0], offsets.numel() - 1
+    if codes.dtype != torch.uint8 or codes.dim() != 2 or codes.shape[1] != M or codebooks.dtype != torch.float32:
+        raise ValueError("codes must be uint8 [T,M] and codebooks fp32 [M,K,d/M]")
+    if scores is None:
+        scores = torch.empty((Q, B), dtype=torch.float32, device=queries.device)
+    lib = load()
+    need = int(lib.tms_maxsim_workspace_bytes(Q, Nq, d, B, _DTYPES[queries.dtype]))
+    if workspace is None and need:
+        workspace = torch.empty(need, dtype=torch.uint8, device=queries.device)
+    ws_ptr = _dev(workspace, "workspace") if workspace is not None else None
+    ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    st = lib.tms_pq_maxsim_decode(_dev(queries, "queries"), Q, Nq, d, _DTYPES[queries.dtype],
+                                  _dev(codebooks, "codebooks"), M, K, _dev(codes, "codes") if T else None,
+                                  _dev(offsets, "offsets"), B, T, _dev(scores, "scores") if B else None, ws_ptr, ws_len,
+                                  _stream(stream))
+    _check(st, "tms_pq_maxsim_decode")
     return scores
 
 

@@ -99,3 +99,43 @@ def test_host_entry_point():
     ws = torch.empty(need + (2 << 20), dtype=torch.uint8, device=DEV)  # ~1 MB per chunk buffer: several chunks
     tms.tms_pq_maxsim_host(q, C, codes.pin_memory(), torch.from_numpy(off), scores, ws)
     assert np.array_equal(scores.numpy().astype(np.float64), ref)
+
+
+# ---- NEXT-4: decode-and-contract variant (codebook resident in shared memory, tensor cores) ---------------------------
+
+def run_decode(q, C, codes, off):
+    out = tms.tms_pq_maxsim_decode(q.to(DEV), C.to(DEV), codes.to(DEV), torch.from_numpy(off).to(DEV))
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("q_dtype", [torch.bfloat16, torch.float16, torch.float32])
+@pytest.mark.parametrize("Q", [1, 8, 11])
+def test_decode_variant_matches_the_oracle_and_the_lut_path(q_dtype, Q):
+    lens = np.concatenate([[5, 128, 1, 0, 300, 16, 17, 15, 0, 0, 33, 1000],
+                           synth.lognormal_lengths(1500, seed=Q, median=60, lo=0, hi=200)])
+    off = synth.offsets_from_lengths(lens)
+    q, C, codes = pq_case(Q, 32, 16, 256, 8, off, seed=20 + Q, q_dtype=q_dtype)
+    got = run_decode(q, C, codes, off)
+    ref = oracle.pq_maxsim(q, C, codes, off)
+    assert_close(got, ref, 2e-3 * 32)
+    fin = np.isfinite(ref)
+    assert np.abs(got[fin] - ref[fin]).max() < 2e-4  # hi/lo split: far inside the tolerance
+    _, lut_scores = run_pq(q, C, codes, off)
+    assert np.abs(got[fin] - lut_scores[fin]).max() < 2e-4
+
+
+def test_decode_variant_exact_on_integer_codebooks():
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(800, seed=4))
+    Q, Nq = 4, 32
+    q = synth.small_int_tokens(Q * Nq, 128, torch.bfloat16, seed=1).view(Q, Nq, 128)
+    C = torch.randint(-2, 3, (16, 256, 8), generator=torch.Generator().manual_seed(3)).to(torch.float32)
+    codes = synth.pq_codes(int(off[-1]), 16, seed=5)
+    assert np.array_equal(run_decode(q, C, codes, off), oracle.pq_maxsim(q, C, codes, off))
+
+
+def test_decode_variant_rejects_other_shapes():
+    off = synth.uniform_offsets(4, 8)
+    q, C, codes = pq_case(1, 8, 8, 64, 4, off, seed=1)
+    with pytest.raises(RuntimeError, match="unsupported"):
+        tms.tms_pq_maxsim_decode(q.to(DEV), C.to(DEV), codes.to(DEV), torch.from_numpy(off).to(DEV))
