@@ -432,7 +432,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     // layout: [operand stages: NS * KBS*16 KB] [F32: raw stages: NR * 32 KB] [SegInfo x NSEG] [park buffers] [barriers]
     constexpr uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
     constexpr uint32_t raw_bytes = PQD ? BN * 16u : 2u * KB_TILE_BYTES;  // PQD: 16 code bytes per token
-    constexpr uint32_t cb_bytes = PQD ? 16u * 256u * 8u * 4u : 0u;        // PQD: the codebook, [16][256][8] fp32
+    constexpr uint32_t cb_bytes = PQD ? 16u * 256u * 8u * 4u : 0u;        // PQD: the codebook [16][256][8], as two bf16 planes
     constexpr int n_epi_warps = 4 * MB;
     uint8_t* st_ptr = smem;
     uint8_t* rw_ptr = st_ptr + (size_t)p.NS * stage_bytes;
@@ -448,8 +448,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint64_t* sempty = sfull + NSEG;             // [NSEG] epilogue -> segmenter
     uint64_t* rfull = sempty + NSEG;             // [NR]   F32: TMA -> splitter
     uint64_t* rempty = rfull + MAX_RAW;          // [NR]   F32: splitter -> TMA (4 warps)
-    uint64_t* cbfull = rempty + MAX_RAW;         // [1]    PQD: the codebook has landed in shared memory
-    uint64_t* aready = cbfull + 1;               // [1]    query rows are in TMEM
+    uint64_t* aready = rempty + MAX_RAW;         // [1]    query rows are in TMEM
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(aready + 1);
     int64_t* range = reinterpret_cast<int64_t*>(aready + 2);  // b_lo, b_hi, t_lo, t_hi
 
@@ -470,7 +469,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
             for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), n_epi_warps); }
             mbar_init(smem_u32(aready), n_epi_warps);
-            mbar_init(smem_u32(cbfull), 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             if (!PQD) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
         }
@@ -507,17 +505,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint64_t pol_docs = policy_evict_first();  // streamed once
         uint32_t s = 0, ph = 0;  // ring slot and its phase bit (F32: the raw ring)
         const uint32_t nring = F32 ? (uint32_t)p.NR : (uint32_t)p.NS;
-        if constexpr (PQD) {
-            if (elect_one()) {  // the codebook, once: 128 KB in four bulk copies
-                mbar_expect_tx(smem_u32(cbfull), cb_bytes);
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    bulk_load(smem_u32(cb_ptr + k * (cb_bytes / 4)),
-                              reinterpret_cast<const uint8_t*>(p.codebooks) + k * (cb_bytes / 4), cb_bytes / 4,
-                              smem_u32(cbfull));
-            }
-            __syncwarp();
-        }
         for (int64_t t = 0; PQD && t < ntiles; ++t) {  // one raw stage per tile: the tile's code rows
             const int64_t tok = t_lo + t * BN;
             const uint32_t bytes = (uint32_t)((p.T - tok < BN ? p.T - tok : BN) * 16);
@@ -701,8 +688,23 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         uint32_t s = 0, ph = 0, rs = 0, rph = 0;
         const int64_t nunits = ntiles * nchunks;
         if constexpr (PQD) {
-            // decode: token row r's 16 codes -> per 64-dimension unit, eight centroid slices of 8 fp32 from the codebook
-            mbar_wait(smem_u32(cbfull), 0);
+            // The codebook goes to shared memory once per CTA, already split: plane 0 holds every centroid slice's
+            // eight bf16 hi parts (16 bytes per (m, k)), plane 1 the lo parts.  Decoding a token is then a pure gather:
+            // token row r's 16 codes -> per 64-dimension unit, eight 16-byte hi pieces and eight lo pieces.
+            {
+                const uint4* g = reinterpret_cast<const uint4*>(p.codebooks);
+                for (int e = r; e < 16 * 256; e += 128) {
+                    const uint4 y0 = ldg_nc16(g + 2 * e), y1 = ldg_nc16(g + 2 * e + 1);
+                    uint4 hi, lo;
+                    split_pair(__uint_as_float(y0.x), __uint_as_float(y0.y), hi.x, lo.x);
+                    split_pair(__uint_as_float(y0.z), __uint_as_float(y0.w), hi.y, lo.y);
+                    split_pair(__uint_as_float(y1.x), __uint_as_float(y1.y), hi.z, lo.z);
+                    split_pair(__uint_as_float(y1.z), __uint_as_float(y1.w), hi.w, lo.w);
+                    *reinterpret_cast<uint4*>(cb_ptr + e * 16) = hi;
+                    *reinterpret_cast<uint4*>(cb_ptr + cb_bytes / 2 + e * 16) = lo;
+                }
+                asm volatile("bar.sync 1, 128;" ::: "memory");  // the four splitter warps
+            }
             for (int64_t t = 0; t < ntiles; ++t) {
                 mbar_wait(smem_u32(rfull + rs), rph);
                 const uint4 cw = *reinterpret_cast<const uint4*>(rw_ptr + (size_t)rs * raw_bytes + r * 16);
@@ -714,14 +716,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     for (int oc = 0; oc < 8; ++oc) {  // sub-quantiser m = 8*ch + oc fills 16-byte piece oc of the unit
                         const uint32_t wsel = ch == 0 ? (oc < 4 ? cword[0] : cword[1]) : (oc < 4 ? cword[2] : cword[3]);
                         const uint32_t code = (wsel >> (8 * (oc & 3))) & 0xffu;
-                        const uint8_t* e = cb_ptr + ((size_t)((8 * ch + oc) * 256 + code) << 5);
-                        const float4 x0 = *reinterpret_cast<const float4*>(e);
-                        const float4 x1 = *reinterpret_cast<const float4*>(e + 16);
-                        uint4 hi, lo;
-                        split_pair(x0.x, x0.y, hi.x, lo.x);
-                        split_pair(x0.z, x0.w, hi.y, lo.y);
-                        split_pair(x1.x, x1.y, hi.z, lo.z);
-                        split_pair(x1.z, x1.w, hi.w, lo.w);
+                        const uint8_t* e = cb_ptr + ((size_t)((8 * ch + oc) * 256 + code) << 4);
+                        const uint4 hi = *reinterpret_cast<const uint4*>(e);
+                        const uint4 lo = *reinterpret_cast<const uint4*>(e + cb_bytes / 2);
                         const uint32_t o = ((uint32_t)oc ^ sw) << 4;
                         *reinterpret_cast<uint4*>(op + o) = hi;
                         *reinterpret_cast<uint4*>(op + KB_TILE_BYTES + o) = lo;

@@ -126,3 +126,10 @@ def test_config4_fused_pq():
     assert err <= 2e-3 * Nq, f"max |dscore| = {err:.3e}"
     ranking_rule(got, ref, 2e-3 * Nq)
     assert 28.0 < got.mean() < 31.0  # sanity range of configs[4]
+    # NEXT-4: the decode-and-contract variant at the same full size, against the same oracle sample and the LUT path
+    dec_d = tms.tms_pq_maxsim_decode(q, C.to(DEV), codes, off_d)
+    torch.cuda.synchronize()
+    dec = dec_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
+    assert np.abs(dec - ref).max() <= 2e-3 * Nq
+    ranking_rule(dec, ref, 2e-3 * Nq)
+    assert float((dec_d - got_d).abs().max()) < 5e-4  # all 8,000,000 scores agree with the LUT path
