@@ -94,7 +94,7 @@ pq_simt_kernel(const float* __restrict__ lut, int Q, int Nq, int M, int K, const
 constexpr int PQS_M = 16, PQS_K = 256, PQS_ROWS = 8;
 constexpr int PQS_SLICE_FLOATS = PQS_ROWS * PQS_M * PQS_K;  // 32768 floats = 128 KB
 constexpr int PQS_SLICE_BYTES = PQS_SLICE_FLOATS * 4;
-constexpr int PQS_WARPS = 16, PQS_THREADS = PQS_WARPS * 32;
+constexpr int PQS_WARPS = 24, PQS_THREADS = PQS_WARPS * 32;
 constexpr int PQS_MAX_SC_FLOATS = 20480;  // 80 KB of per-chunk score accumulators
 
 // lut [R, 16, 256] -> lutT [R/8 slices][4 g][256 k][4 sub][8 rows]
