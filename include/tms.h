@@ -72,10 +72,10 @@ typedef enum {
  * total_tokens  = offsets[B]; passed by value so the host never reads device memory.
  * scores        device, fp32 [Q, B] row-major, overwritten.
  * workspace     device scratch of at least tms_maxsim_workspace_bytes(...) bytes, 16-byte aligned; may be
- *               NULL when that size is 0 (it is 0 for Nq <= 32).  Queries of Nq = 64, 96, ... tokens are
- *               scored as 32-token parts whose partial scores (fp32 [Q*Nq/32, B]) live in the workspace
- *               and are added by a second kernel; without the workspace such shapes take the general
- *               CUDA-core kernel.
+ *               NULL when that size is 0 (it is 0 for Nq <= 32).  Longer queries are scored as n equal parts
+ *               of Nq/n <= 32 tokens (n = Nq/32 for multiples of 32) whose partial scores (fp32 [Q*n, B])
+ *               live in the workspace and are added by a second kernel; without the workspace such shapes
+ *               take the general CUDA-core kernel.
  * Every document embedding is read from HBM once per group of up to 256 query rows (Q*Nq, with Nq
  * rounded up to a power of two); no similarity matrix is written to memory (Eq. 7).
  * d > 128 accumulates partial dot products over dimension chunks before the max is taken.

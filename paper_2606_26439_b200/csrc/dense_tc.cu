@@ -1012,12 +1012,20 @@ int next_pow2(int v) {
     return p;
 }
 
+// Number of equal parts a query of Nq tokens is scored in: the smallest n with Nq % n == 0 and Nq / n <= 32
+// (1 for Nq <= 32; Nq / 32 for multiples of 32; 2 x 24 for Nq = 48; Nq parts of one token for a prime Nq > 32).
+int query_parts(int Nq) {
+    for (int n = 1; n <= Nq; ++n)
+        if (Nq % n == 0 && Nq / n <= 32) return n;
+    return Nq;
+}
+
 struct Plan {
     Params p;           // per-launch fields (queries, scores, Q) are filled in by the launcher
     int MB, KBS;        // query blocks per launch, dimension blocks per stage
     bool f32;           // fp32 inputs: split into bf16 pairs on the fly
     bool pqd;           // decode-and-contract PQ variant
-    int nparts;         // 32-token parts per query (1 unless Nq > 32)
+    int nparts;         // equal parts a query is scored in (1 unless Nq > 32)
     int Qg;             // queries per launch
     uint32_t smem_bytes;
 };
@@ -1038,13 +1046,13 @@ bool plan(const DenseArgs& a, Plan& pl) {
     const int row_bytes = a.d * esize;  // of a query row; also of a document row unless pqd
     // 16-bit: whole 128-byte dimension blocks; fp32: whole 64-element units (256 bytes)
     if (!pqd && row_bytes % (f32 ? 2 * KB_BYTES : KB_BYTES) != 0) return false;
-    // A query's rows must sit inside one warp's 32 TMEM lanes.  Longer queries (Nq a multiple of 32) are scored as
-    // Nq/32 parts of 32 tokens -- queries[Q,Nq,d] read as [Q*Nq/32, 32, d] -- into a workspace of partial scores that
+    // A query's rows must sit inside one warp's 32 TMEM lanes.  Longer queries are scored as n equal parts of Nq/n <= 32
+    // tokens -- queries[Q,Nq,d] read as [Q*n, Nq/n, d] -- into a workspace of partial scores that
     // sum_parts_kernel adds up (Eq. 1's outer sum is associative over query tokens, pin P9).
-    const int nparts = a.Nq > 32 ? a.Nq / 32 : 1;
-    if (a.Nq > 32 && (a.Nq % 32 != 0 || !a.workspace || a.workspace_bytes < dense_tc_workspace_bytes(a.Q, a.Nq, a.B)))
-        return false;
-    const int Nq_part = nparts > 1 ? 32 : a.Nq;
+    const int nparts = query_parts(a.Nq);
+    if (nparts > 1 && (!a.workspace || a.workspace_bytes < dense_tc_workspace_bytes(a.Q, a.Nq, a.B))) return false;
+    if ((int64_t)a.Q * nparts > (1 << 20)) return false;
+    const int Nq_part = a.Nq / nparts;
     const int nqp = next_pow2(Nq_part);
     const int NKB = f32 ? a.d / 64 : row_bytes / KB_BYTES;  // fp32: 64-element units
     // TMEM budget: query rows (fp32: bf16 hi and lo halves) + at least MB accumulators of 128 columns
@@ -1109,8 +1117,8 @@ bool plan(const DenseArgs& a, Plan& pl) {
 }  // namespace
 
 size_t dense_tc_workspace_bytes(int Q, int Nq, int64_t B) {
-    if (Nq <= 32 || Nq % 32 != 0) return 0;
-    return sizeof(float) * (size_t)Q * (size_t)(Nq / 32) * (size_t)B;
+    if (Nq <= 32) return 0;
+    return sizeof(float) * (size_t)Q * (size_t)query_parts(Nq) * (size_t)B;
 }
 
 bool dense_tc_supports(const DenseArgs& a) {

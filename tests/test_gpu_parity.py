@@ -158,7 +158,7 @@ def test_p11_zero_padded_dimensions_tie_the_tiled_variant_to_d128():
 
 # ---- NEXT-1 shapes: the paper's Nq sweep (Table 10) and Nd sweep (Table 11) -----------------
 
-@pytest.mark.parametrize("Nq", [8, 16, 64, 96])
+@pytest.mark.parametrize("Nq", [8, 16, 37, 48, 64, 96])
 def test_query_length_sweep(Nq):
     off = synth.offsets_from_lengths(np.concatenate([RAGGED, synth.lognormal_lengths(1500, seed=Nq)]))
     q, D = unit_case(3, Nq, 128, torch.bfloat16, off, seed=40 + Nq)
