@@ -818,7 +818,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
 #pragma unroll
                     for (int j = 0; j < KB_WORDS / 4; ++j) {
                         uint4 x = make_uint4(0, 0, 0, 0);
-                        if (row_valid) x = ldg_nc16(src + kb * KB_BYTES + j * 16);
+                        if (row_valid && kb * KB_BYTES + j * 16 < p.row_bytes) x = ldg_nc16(src + kb * KB_BYTES + j * 16);
                         w[4 * j] = x.x; w[4 * j + 1] = x.y; w[4 * j + 2] = x.z; w[4 * j + 3] = x.w;
                     }
                     tmem_st32(lane_addr + (uint32_t)((mb * p.NKB + kb) * KB_WORDS), w);
@@ -1044,8 +1044,9 @@ bool plan(const DenseArgs& a, Plan& pl) {
     const bool f32 = pqd || a.dtype == TMS_DTYPE_F32;
     const int esize = (int)dtype_size(a.dtype);
     const int row_bytes = a.d * esize;  // of a query row; also of a document row unless pqd
-    // 16-bit: whole 128-byte dimension blocks; fp32: whole 64-element units (256 bytes)
-    if (!pqd && row_bytes % (f32 ? 2 * KB_BYTES : KB_BYTES) != 0) return false;
+    // fp32: whole 64-element units (256 bytes).  16-bit: any 16-byte multiple -- TMA zero-fills the part of the last
+    // 128-byte dimension block that lies beyond the row, and the query rows are zero-padded the same way.
+    if (!pqd && row_bytes % (f32 ? 2 * KB_BYTES : 16) != 0) return false;
     // A query's rows must sit inside one warp's 32 TMEM lanes.  Longer queries are scored as n equal parts of Nq/n <= 32
     // tokens -- queries[Q,Nq,d] read as [Q*n, Nq/n, d] -- into a workspace of partial scores that
     // sum_parts_kernel adds up (Eq. 1's outer sum is associative over query tokens, pin P9).
@@ -1054,7 +1055,7 @@ bool plan(const DenseArgs& a, Plan& pl) {
     if ((int64_t)a.Q * nparts > (1 << 20)) return false;
     const int Nq_part = a.Nq / nparts;
     const int nqp = next_pow2(Nq_part);
-    const int NKB = f32 ? a.d / 64 : row_bytes / KB_BYTES;  // fp32: 64-element units
+    const int NKB = f32 ? a.d / 64 : (row_bytes + KB_BYTES - 1) / KB_BYTES;  // fp32: 64-element units
     // TMEM budget: query rows (fp32: bf16 hi and lo halves) + at least MB accumulators of 128 columns
     const int a_cols_per_block = (f32 ? 2 : 1) * NKB * KB_WORDS;
     int MB = 2;

@@ -227,6 +227,16 @@ def test_host_entry_point_streams_chunks():
         tms.tms_maxsim_host(q, D, torch.from_numpy(off), scores, small)
 
 
+@pytest.mark.parametrize("d", [8, 32, 48, 80, 96, 160, 200])
+def test_dimensions_that_are_not_whole_128_byte_blocks(d):
+    off = synth.offsets_from_lengths(np.concatenate([RAGGED, synth.lognormal_lengths(700, seed=d)]))
+    q, D = unit_case(5, 32, d, torch.bfloat16, off, seed=80 + d)
+    assert_close(run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
+    qi = synth.small_int_tokens(5 * 32, d, torch.float16, seed=5).view(5, 32, d)
+    Di = synth.small_int_tokens(int(off[-1]), d, torch.float16, seed=6)
+    assert np.array_equal(run_dense(qi, Di, off, "tcgen05"), oracle.maxsim(qi, Di, off))
+
+
 # ---- randomised shapes: every path of the tcgen05 kernel against the oracle --------------------------------------------
 
 def _fuzz_lengths(rng, B):
