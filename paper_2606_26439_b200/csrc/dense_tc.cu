@@ -14,15 +14,16 @@
 //   D          S = Qmat . D_tile^T in TMEM, fp32, one 128-lane x 128-column accumulator per 128 query rows, in
 //              a ring of accumulators.  For d*sizeof > one stage the MMAs of successive dimension chunks
 //              accumulate into the same accumulator; the max is taken once after the last chunk
-//   epilogue   tcgen05.ld (32 columns at a time, the next load in flight while the current columns are
-//              reduced) -> running max per query row, segmented by document with a carry across tiles
-//              (Alg. 3 line 8).  At a document's last token each row parks its maximum in a small per-warp
-//              shared-memory buffer; every 16 documents the warp sums the Nq maxima of each query in ascending
-//              row order and stores 16 scores                                                        (Eq. 1)
+//   epilogue   tcgen05.ld of 32 accumulator columns per thread at a time (pipelined against the reduction when two
+//              epilogue warps share a scheduler) -> running max per query row, segmented by document with a carry
+//              across tiles (Alg. 3 line 8).  At a document's last token each row parks its maximum in a small
+//              per-warp shared-memory buffer; when 16 documents are parked the warp adds the Nq maxima of each
+//              query in a fixed order and stores 16 scores                                           (Eq. 1)
 //
-// Warp roles (blockDim = 128 + 128*MB): warp 0 TMA producer, warp 1 MMA issuer + TMEM owner, warp 2 document
-// segmenter (turns `offsets` into per-tile boundary masks, writes -inf for empty documents), warp 3 idle,
-// warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of query block (w-4)/4).
+// Warp roles (blockDim = 128 + 128*MB, + 128 for the split paths): warp 0 TMA producer, warp 1 MMA issuer + TMEM
+// owner, warp 2 document segmenter (turns `offsets` into per-tile boundary masks, writes -inf for empty documents),
+// warp 3 idle, warps 4.. epilogue (warp w reads TMEM lanes 32*(w%4)..+31 of query block (w-4)/4), and for fp32 inputs
+// / PQ codes four more warps that turn what TMA lands into bf16 hi/lo operand stages (see the kernel's comment).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
