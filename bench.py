@@ -49,6 +49,9 @@ WORKLOADS = {
     "n1-nq8": dict(kind="dense", Q=1, Nq=8, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "n1-nq16": dict(kind="dense", Q=1, Nq=16, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "n1-nq64": dict(kind="dense", Q=1, Nq=64, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    "n1-b1k": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=1_000, Nd=128, lengths="uniform"),
+    "n1-b10k": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=10_000, Nd=128, lengths="uniform"),
+    "n1-b100k": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "n1-nd32": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=32, lengths="uniform"),
     "n1-nd64": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=64, lengths="uniform"),
     "n1-nd256": dict(kind="dense", Q=1, Nq=32, d=128, dtype="bf16", B=100_000, Nd=256, lengths="uniform"),
