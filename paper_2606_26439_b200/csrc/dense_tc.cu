@@ -68,9 +68,28 @@ struct Params {
     const float* codebooks;
     int q_fmt;             // element type of the query rows: 0 fp32, 1 fp16, 2 bf16 (fp32-split paths only)
     int skip_alo;          // the queries' lo halves are all zero (bf16 queries): leave out the a_lo * b_hi MMAs
-    int debug;             // TMS_DEBUG bits (measurement probes only): 1 skip epilogue math, 2 skip MMAs, 4 skip TMEM
-                           // reads, 8 write the SM clock seen by each CTA over two scores
+#ifdef TMS_PROBES
+    const void* docs_raw;
+    int debug;             // probe builds only (-DTMS_PROBES, never set by build.py): TMS_DEBUG bits 1 skip epilogue
+                           // math, 2 skip MMAs, 4 skip TMEM reads.  The product library has none of this.
+#endif
 };
+
+// Measurement probes exist only in builds made with -DTMS_PROBES (a separate library for experiments; build.py never
+// sets it): skip switches read from the environment, and a per-role clock trace of one CTA.
+#ifdef TMS_PROBES
+#define PROBE(p, bit) (((p).debug & (bit)) != 0)
+constexpr int TRACE_NT = 64, TRACE_T0 = 200, TRACE_CTA = 5, TRACE_EV = 8, TRACE_ROLES = 4;
+__device__ long long g_trace[TRACE_ROLES * TRACE_NT * TRACE_EV];
+#define TRACE(role, t, ev)                                                                                    \
+    do {                                                                                                      \
+        if (blockIdx.x == TRACE_CTA && lane == 0 && (t) >= TRACE_T0 && (t) < TRACE_T0 + TRACE_NT)             \
+            g_trace[((role) * TRACE_NT + (int)((t) - TRACE_T0)) * TRACE_EV + (ev)] = clock64();               \
+    } while (0)
+#else
+#define PROBE(p, bit) false
+#define TRACE(role, t, ev) do { } while (0)
+#endif
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -454,12 +473,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     int64_t* range = reinterpret_cast<int64_t*>(aready + 2);  // b_lo, b_hi, t_lo, t_hi
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    uint64_t dbg_g0 = 0;
-    long long dbg_c0 = 0;
-    if (p.debug & 8) {
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_g0));
-        dbg_c0 = clock64();
-    }
 
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0) {
@@ -531,6 +544,15 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     }
                 } else {
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
+                    if (ch == 0) TRACE(0, t, 0);
+#ifdef TMS_PROBES
+                    if (PROBE(p, 8)) {  // probe: one linear 1-D bulk copy per stage instead of the 2-D tensor copies (wrong data layout, timing only)
+                        if (elect_one()) {
+                            mbar_expect_tx(smem_u32(full + s), stage_bytes);
+                            bulk_load(smem_u32(st_ptr + (size_t)s * stage_bytes), (const uint8_t*)p.docs_raw + (size_t)tok * p.row_bytes, stage_bytes, smem_u32(full + s));
+                        }
+                    } else
+#endif
                     if (elect_one()) {
                         mbar_expect_tx(smem_u32(full + s), stage_bytes);
 #pragma unroll
@@ -540,6 +562,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     }
                 }
                 __syncwarp();
+                if (ch == nchunks - 1) TRACE(0, t, 2);
                 if (++s == nring) { s = 0; ph ^= 1; }
             }
         }
@@ -552,7 +575,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         tc_fence_after();
         const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
         const uint32_t idesc = p.idesc;
-        const bool skip = (p.debug & 2) != 0, skip_alo = p.skip_alo != 0;
+        const bool skip = PROBE(p, 2), skip_alo = p.skip_alo != 0;
         const uint32_t nacc = (uint32_t)p.NACC;
         const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
         // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
@@ -566,14 +589,25 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         for (int64_t t = 0; t < ntiles; ++t) {
             uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
             for (int ch = 0; ch < nchunks; ++ch) {
+                if (ch == 0) TRACE(1, t, 5);
                 mbar_wait(smem_u32(full + s), ph);
+                if (ch == 0) TRACE(1, t, 6);
                 tc_fence_after();
+                if (ch == 0) TRACE(1, t, 0);
+#ifdef TMS_PROBES
+                if (ch == 0 && blockIdx.x == TRACE_CTA && lane == 0 && t >= TRACE_T0 && t < TRACE_T0 + TRACE_NT) {
+                    uint64_t g;
+                    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
+                    g_trace[(1 * TRACE_NT + (int)(t - TRACE_T0)) * TRACE_EV + 7] = (long long)g;
+                }
+#endif
                 const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
 #pragma unroll
                 for (int mb = 0; mb < MB; ++mb) {
                     if (ch == 0) {  // the epilogue has drained this accumulator
                         mbar_wait(smem_u32(tempty + slot[mb]), tph[mb] ^ 1);
                         tc_fence_after();
+                        TRACE(1, t, 1 + 2 * mb);
                     }
                     const uint32_t d_tmem = acc0 + slot[mb] * BN;
                     if (elect_one()) {
@@ -611,6 +645,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         if (mb == MB - 1 && !epi_frees_stage) tc_commit(smem_u32(empty + s));
                     }
                     __syncwarp();
+                    if (ch == nchunks - 1) TRACE(1, t, 2 + 2 * mb);
                 }
                 a_col += (F32 ? 1 : KBS) * KB_WORDS;
                 if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
@@ -680,6 +715,18 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // documents after the last token of the range can only be empty
         for (int64_t idx = wb + consumed + lane; idx < b_hi; idx += 32)
             for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
+#ifdef TMS_PROBES
+    } else if (warp == 3 && !F32) {
+        // probe: observer of the `full` barriers (when does each tile's data land?) -- role 0, events 1..
+        uint32_t s = 0, ph = 0;
+        for (int64_t t = 0; t < ntiles; ++t) {
+            for (int ch = 0; ch < nchunks; ++ch) {
+                mbar_wait(smem_u32(full + s), ph);
+                if (ch == nchunks - 1) TRACE(0, t, 1);
+                if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
+            }
+        }
+#endif
     } else if (F32 && warp >= 4 + n_epi_warps) {
         // ===== fp32 splitter (F32 only): raw fp32 stage -> bf16 hi block + bf16 lo block of an operand stage =====
         // Thread r owns token row r of the tile.  Both layouts are the 128-byte swizzle (16-byte piece index XOR
@@ -838,7 +885,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t cfg = pack_cfg(p.Nq, p.Nq_pad, nvalid);
         float* out = p.scores + (int64_t)q0 * p.B + b_lo;
         const uint32_t pend = smem_u32(pend_all) + (uint32_t)ew * (PEND_IDS + PEND * 4);
-        const bool skip_math = (p.debug & 1) != 0;
+        const bool skip_math = PROBE(p, 1);
         const int64_t B = p.B;
         const bool frees_stage = !F32 && nchunks == 1 && ew == 4 * (MB - 1);  // see the MMA warp
 
@@ -850,14 +897,16 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t acc0 = lane_addr + (uint32_t)p.acc_col0;
         uint32_t slot = (uint32_t)mb, tph = 0, g = 0, gph = 0, rs = 0;
         for (int64_t t = 0; t < ntiles; ++t) {
+            if (quad == 0) TRACE(2 + mb, t, 0);
             mbar_wait(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb), (uint32_t)(t >> 2) & 1u);
             tc_fence_after();
+            if (quad == 0) TRACE(2 + mb, t, 1);
             if (frees_stage) {  // the tile's only stage has been read by the tensor pipe: back to the producer
                 if (lane == 0) mbar_arrive(smem_u32(empty + rs));
                 if (++rs == (uint32_t)p.NS) rs = 0;
             }
             const uint32_t taddr = acc0 + slot * BN;
-            if (p.debug & 4) {  // measurement probe: no TMEM reads at all
+            if (PROBE(p, 4)) {  // measurement probe: no TMEM reads at all
                 mbar_wait(smem_u32(sfull + g), gph);
                 tc_fence_before();
                 __syncwarp();
@@ -901,19 +950,24 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
                 st.k = 0;
                 tmem_ld_wait32(va);
+                if (quad == 0) TRACE(2 + mb, t, 2);
                 tmem_ld32(taddr + 32, vb);
                 process32(va, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
                 tmem_ld_wait32(vb);
+                if (quad == 0) TRACE(2 + mb, t, 3);
                 tmem_ld32(taddr + 64, va);
                 process32(vb, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
                 tmem_ld_wait32(va);
+                if (quad == 0) TRACE(2 + mb, t, 4);
                 tmem_ld32(taddr + 96, vb);
                 process32(va, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
                 tmem_ld_wait32(vb);
+                if (quad == 0) TRACE(2 + mb, t, 5);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
                 process32(vb, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
+                if (quad == 0) TRACE(2 + mb, t, 6);
             } else {
                 // One epilogue warp per scheduler: every extra tcgen05.wait::ld costs more than the overlap gains, so the
                 // whole accumulator is loaded at once and handed back to the MMA warp before any of it is reduced.
@@ -950,12 +1004,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     // ---- teardown --------------------------------------------------------------------------------------------
     tc_fence_before();
     __syncthreads();
-    if ((p.debug & 8) && threadIdx.x == 0) {  // measurement probe: SM clock seen by this CTA (overwrites two scores)
-        uint64_t g1;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
-        p.scores[2 * blockIdx.x] = (float)(clock64() - dbg_c0);
-        p.scores[2 * blockIdx.x + 1] = (float)(g1 - dbg_g0);
-    }
     if (warp == 1) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)TMEM_COLS)
@@ -1080,10 +1128,13 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.NACC = (TMEM_COLS - MB * a_cols_per_block) / BN;
     if (p.NACC > MAX_ACC) p.NACC = MAX_ACC;
     p.acc_col0 = TMEM_COLS - p.NACC * BN;
-    {   // measurement probes, read once per process; 0 in every reported number
+#ifdef TMS_PROBES
+    {
         static const int dbg = [] { const char* e = getenv("TMS_DEBUG"); return e ? atoi(e) & 15 : 0; }();
         p.debug = dbg;
+        p.docs_raw = a.docs;
     }
+#endif
     const uint32_t fmt = (!f32 && a.dtype == TMS_DTYPE_F16) ? 0u : 1u;  // the split paths feed bf16 pairs
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
@@ -1118,6 +1169,14 @@ bool plan(const DenseArgs& a, Plan& pl) {
 
 }  // namespace
 
+#ifdef TMS_PROBES
+// probe builds only: copies the clock trace of CTA TRACE_CTA to the host ([role][tile][event])
+extern "C" int tms_trace_read(long long* host, int* roles, int* tiles, int* events) {
+    *roles = TRACE_ROLES; *tiles = TRACE_NT; *events = TRACE_EV;
+    return cudaMemcpyFromSymbol(host, g_trace, sizeof(long long) * TRACE_ROLES * TRACE_NT * TRACE_EV) == cudaSuccess ? 0 : 1;
+}
+#endif
+
 size_t dense_tc_workspace_bytes(int Q, int Nq, int64_t B) {
     if (Nq <= 32) return 0;
     return sizeof(float) * (size_t)Q * (size_t)query_parts(Nq) * (size_t)B;
@@ -1151,6 +1210,10 @@ int launch_dense_tc(const DenseArgs& a) {
     // no more CTAs than 128-token tiles; one CTA per SM
     int64_t grid = (a.T + BN - 1) / BN;
     if (grid > di->num_sms) grid = di->num_sms;
+#ifdef TMS_PROBES
+    if (const char* e = getenv("TMS_GRID")) { const int g = atoi(e); if (g > 0 && g < grid) grid = g; }
+    if (const char* e = getenv("TMS_NS")) { const int n = atoi(e); if (n > 0 && n < pl.p.NS) pl.p.NS = n; }
+#endif
     // one launch per group of Qg queries (up to 256 query rows): the store is streamed once per group
     const int Qeff = a.Q * pl.nparts;  // queries as the kernel sees them (32-token parts of long queries)
     float* dst = pl.nparts > 1 ? static_cast<float*>(a.workspace) : a.scores;
