@@ -86,9 +86,16 @@ __device__ long long g_trace[TRACE_ROLES * TRACE_NT * TRACE_EV];
         if (blockIdx.x == TRACE_CTA && lane == 0 && (t) >= TRACE_T0 && (t) < TRACE_T0 + TRACE_NT)             \
             g_trace[((role) * TRACE_NT + (int)((t) - TRACE_T0)) * TRACE_EV + (ev)] = clock64();               \
     } while (0)
+// same from a region only one thread executes
+#define TRACE1(role, t, ev)                                                                                   \
+    do {                                                                                                      \
+        if (blockIdx.x == TRACE_CTA && (t) >= TRACE_T0 && (t) < TRACE_T0 + TRACE_NT)                          \
+            g_trace[((role) * TRACE_NT + (int)((t) - TRACE_T0)) * TRACE_EV + (ev)] = clock64();               \
+    } while (0)
 #else
 #define PROBE(p, bit) false
 #define TRACE(role, t, ev) do { } while (0)
+#define TRACE1(role, t, ev) do { } while (0)
 #endif
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------
@@ -115,6 +122,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "}\n" ::"r"(bar),
         "r"(parity)
         : "memory");
+}
+// non-blocking: has the phase with this parity completed?
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.b32 %0, 1, 0, p;\n}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
 }
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1,
                                             uint64_t policy) {
@@ -469,8 +486,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint64_t* rfull = sempty + NSEG;             // [NR]   F32: TMA -> splitter
     uint64_t* rempty = rfull + MAX_RAW;          // [NR]   F32: splitter -> TMA (4 warps)
     uint64_t* aready = rempty + MAX_RAW;         // [1]    query rows are in TMEM
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(aready + 1);
-    int64_t* range = reinterpret_cast<int64_t*>(aready + 2);  // b_lo, b_hi, t_lo, t_hi
+    uint64_t* turn = aready + 1;                 // [2]    MMA issuer w may start its next tile (the other one is done issuing)
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(turn + 2);
+    int64_t* range = reinterpret_cast<int64_t*>(turn + 3);  // b_lo, b_hi, t_lo, t_hi
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -483,6 +501,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
             for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), n_epi_warps); }
             mbar_init(smem_u32(aready), n_epi_warps);
+            mbar_init(smem_u32(turn), 1);
+            mbar_init(smem_u32(turn + 1), 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             if (!PQD) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
         }
@@ -566,51 +586,68 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 if (++s == nring) { s = 0; ph ^= 1; }
             }
         }
-    } else if (warp == 1) {
-        // ===== MMA issuer =====
-        // One elected lane issues every tcgen05.mma of the CTA (the whole warp follows the barriers), so its
-        // instruction stream must stay short: the loops over K steps and query blocks are compile-time, and a
-        // descriptor is the previous one plus a constant.
+    } else if (warp == 1 || warp == 3) {
+        // ===== MMA issuers =====
+        // Two warps issue alternate tiles (warp 1 the even ones, warp 3 the odd ones).  Why two: the thread that issues
+        // tcgen05.mma blocks while the MMA queue is full, so it reaches the code after a tile's last MMA with only a
+        // few MMAs (~250 clk of tensor work) still queued; the barrier waits, ring arithmetic and descriptor set-up
+        // of the next tile take a lone warp longer than that and the tensor pipe ran dry at every tile boundary
+        // (traced: 1,024 clk of MMAs per 1,380 clk tile period).  With two issuers all of that happens while the
+        // other warp is issuing; what is left on the critical path is the hand-over: one mbarrier arrive after the
+        // last MMA of a tile has been accepted, and the waiting warp's wake-up.  MMAs of different tiles are never
+        // interleaved (switching accumulators between consecutive MMAs costs tensor-pipe time).
+        // Inside a tile one elected lane issues everything; the rest of the warp follows the barriers, so the ring
+        // arithmetic stays warp-uniform (uniform datapath, descriptors are the previous one plus a constant).
+        const uint32_t w = (uint32_t)warp >> 1;  // 0: even tiles, 1: odd tiles
         mbar_wait(smem_u32(aready), 0);
         tc_fence_after();
         const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
         const uint32_t idesc = p.idesc;
         const bool skip = PROBE(p, 2), skip_alo = p.skip_alo != 0;
-        const uint32_t nacc = (uint32_t)p.NACC;
+        const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS;
         const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
         // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
         const uint32_t a_lo_off = (uint32_t)p.NKB * KB_WORDS;
         const uint32_t a_mb_step = F32 ? 2 * a_lo_off : a_lo_off;
         const bool epi_frees_stage = !F32 && nchunks == 1;
+        const uint32_t full0 = smem_u32(full), tempty0 = smem_u32(tempty), tfull0 = smem_u32(tfull);
+        const uint32_t my_turn = smem_u32(turn + w), other_turn = smem_u32(turn + (w ^ 1));
+        // ring positions of this warp's first tile (tile w): operand stage w*nchunks, accumulator jobs w*MB + mb
         uint32_t s = 0, ph = 0;
+        for (uint32_t c = 0; c < w * (uint32_t)nchunks; ++c)
+            if (++s == NS) { s = 0; ph ^= 1; }
         uint32_t slot[MB], tph[MB];
 #pragma unroll
-        for (int mb = 0; mb < MB; ++mb) { slot[mb] = mb; tph[mb] = 0; }
-        for (int64_t t = 0; t < ntiles; ++t) {
-            uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
-            for (int ch = 0; ch < nchunks; ++ch) {
-                if (ch == 0) TRACE(1, t, 5);
-                mbar_wait(smem_u32(full + s), ph);
-                if (ch == 0) TRACE(1, t, 6);
-                tc_fence_after();
-                if (ch == 0) TRACE(1, t, 0);
-#ifdef TMS_PROBES
-                if (ch == 0 && blockIdx.x == TRACE_CTA && lane == 0 && t >= TRACE_T0 && t < TRACE_T0 + TRACE_NT) {
-                    uint64_t g;
-                    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
-                    g_trace[(1 * TRACE_NT + (int)(t - TRACE_T0)) * TRACE_EV + 7] = (long long)g;
-                }
-#endif
-                const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
+        for (int mb = 0; mb < MB; ++mb) {
+            slot[mb] = 0; tph[mb] = 0;
+            for (uint32_t c = 0; c < w * MB + (uint32_t)mb; ++c)
+                if (++slot[mb] == nacc) { slot[mb] = 0; tph[mb] ^= 1; }
+        }
+        const bool early_full = NS > (uint32_t)nchunks, early_acc = nacc > (uint32_t)MB;
+        uint32_t tp = 0;  // parity of `turn` to wait for; warp 1's first tile (tile 0) needs no hand-over
+        for (int64_t t = w; t < ntiles; t += 2) {
+            // The tile's first stage and first accumulator are awaited BEFORE the hand-over when that is safe: a
+            // parity wait is only meaningful once the barrier's previous phase has completed, which is certain when
+            // that phase belongs to a tile <= t-2 (issued before this warp's previous hand-over), i.e. when the ring
+            // is longer than one tile's worth (NS > nchunks, NACC > MB).  Otherwise they are awaited after it.
+            if (early_full) mbar_wait(full0 + s * 8, ph);
+            if (early_acc) mbar_wait(tempty0 + slot[0] * 8, tph[0] ^ 1);  // the epilogue has drained block 0's accumulator
+            if (t != 0) { mbar_wait(my_turn, tp); tp ^= 1; }
+            if (!early_full) mbar_wait(full0 + s * 8, ph);
+            if (!early_acc) mbar_wait(tempty0 + slot[0] * 8, tph[0] ^ 1);
+            tc_fence_after();
+            TRACE(1, t, 0);
+            if (elect_one()) {
+                uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
+                uint32_t sc = s, phc = ph;
+                for (int ch = 0; ch < nchunks; ++ch) {
+                    if (ch != 0) { mbar_wait(full0 + sc * 8, phc); tc_fence_after(); }
+                    const uint32_t b_lo = b_lo0 + sc * (stage_bytes >> 4);
+                    const bool last_chunk = ch == nchunks - 1;
 #pragma unroll
-                for (int mb = 0; mb < MB; ++mb) {
-                    if (ch == 0) {  // the epilogue has drained this accumulator
-                        mbar_wait(smem_u32(tempty + slot[mb]), tph[mb] ^ 1);
-                        tc_fence_after();
-                        TRACE(1, t, 1 + 2 * mb);
-                    }
-                    const uint32_t d_tmem = acc0 + slot[mb] * BN;
-                    if (elect_one()) {
+                    for (int mb = 0; mb < MB; ++mb) {
+                        if (ch == 0 && mb != 0) { mbar_wait(tempty0 + slot[mb] * 8, tph[mb] ^ 1); tc_fence_after(); }
+                        const uint32_t d_tmem = acc0 + slot[mb] * BN;
                         if (!skip) {
                             if constexpr (F32) {
 #pragma unroll
@@ -641,19 +678,23 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         // accumulator -> epilogue.  When a tile is a single stage, the last block's barrier also tells
                         // the epilogue that the stage has been read (it hands the stage back to the producer): one
                         // tcgen05.commit fewer per tile.
-                        if (ch == nchunks - 1) tc_commit(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb));
-                        if (mb == MB - 1 && !epi_frees_stage) tc_commit(smem_u32(empty + s));
+                        if (last_chunk) tc_commit(tfull0 + ((uint32_t)(t & 3) * MB + mb) * 8);
+                        if (mb == MB - 1 && !epi_frees_stage) tc_commit(smem_u32(empty + sc));
+                        if (last_chunk && mb == MB - 1) mbar_arrive(other_turn);  // the other issuer may start its tile
                     }
-                    __syncwarp();
-                    if (ch == nchunks - 1) TRACE(1, t, 2 + 2 * mb);
+                    a_col += (F32 ? 1 : KBS) * KB_WORDS;
+                    if (++sc == NS) { sc = 0; phc ^= 1; }
                 }
-                a_col += (F32 ? 1 : KBS) * KB_WORDS;
-                if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
             }
+            __syncwarp();
+            TRACE(1, t, 4);
+            // this warp's next tile is two tiles on
+            for (int c = 0; c < 2 * nchunks; ++c)
+                if (++s == NS) { s = 0; ph ^= 1; }
 #pragma unroll
             for (int mb = 0; mb < MB; ++mb) {
-                slot[mb] += MB;
-                if (slot[mb] >= nacc) { slot[mb] -= nacc; tph[mb] ^= 1; }
+                slot[mb] += 2 * MB;
+                while (slot[mb] >= nacc) { slot[mb] -= nacc; tph[mb] ^= 1; }
             }
         }
     } else if (warp == 2) {
@@ -715,18 +756,6 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // documents after the last token of the range can only be empty
         for (int64_t idx = wb + consumed + lane; idx < b_hi; idx += 32)
             for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
-#ifdef TMS_PROBES
-    } else if (warp == 3 && !F32) {
-        // probe: observer of the `full` barriers (when does each tile's data land?) -- role 0, events 1..
-        uint32_t s = 0, ph = 0;
-        for (int64_t t = 0; t < ntiles; ++t) {
-            for (int ch = 0; ch < nchunks; ++ch) {
-                mbar_wait(smem_u32(full + s), ph);
-                if (ch == nchunks - 1) TRACE(0, t, 1);
-                if (++s == (uint32_t)p.NS) { s = 0; ph ^= 1; }
-            }
-        }
-#endif
     } else if (F32 && warp >= 4 + n_epi_warps) {
         // ===== fp32 splitter (F32 only): raw fp32 stage -> bf16 hi block + bf16 lo block of an operand stage =====
         // Thread r owns token row r of the tile.  Both layouts are the 128-byte swizzle (16-byte piece index XOR
@@ -1082,7 +1111,7 @@ struct Plan {
 uint32_t fixed_smem(int MB) {
     const uint32_t warps = 4u * MB;
     return (uint32_t)sizeof(SegInfo) * NSEG + warps * PEND * (PEND_PITCH + 1) * 4 +
-           8u * (2 * MAX_STAGES + 8 + MAX_ACC + 2 * NSEG + 2 * MAX_RAW + 2) + 4 * 8 + 1024 /* alignment slack */;
+           8u * (2 * MAX_STAGES + 8 + MAX_ACC + 2 * NSEG + 2 * MAX_RAW + 4) + 4 * 8 + 1024 /* alignment slack */;
 }
 
 // Shape -> kernel parameters; false when the tcgen05 path does not cover it.
@@ -1130,7 +1159,7 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.acc_col0 = TMEM_COLS - p.NACC * BN;
 #ifdef TMS_PROBES
     {
-        static const int dbg = [] { const char* e = getenv("TMS_DEBUG"); return e ? atoi(e) & 15 : 0; }();
+        static const int dbg = [] { const char* e = getenv("TMS_DEBUG"); return e ? atoi(e) : 0; }();
         p.debug = dbg;
         p.docs_raw = a.docs;
     }
