@@ -92,10 +92,16 @@ __device__ long long g_trace[TRACE_ROLES * TRACE_NT * TRACE_EV];
         if (blockIdx.x == TRACE_CTA && (t) >= TRACE_T0 && (t) < TRACE_T0 + TRACE_NT)                          \
             g_trace[((role) * TRACE_NT + (int)((t) - TRACE_T0)) * TRACE_EV + (ev)] = clock64();               \
     } while (0)
+#ifdef TMS_TRACE_DETAIL
+#define TRACED(role, t, ev) TRACE(role, t, ev)
+#else
+#define TRACED(role, t, ev) do { } while (0)
+#endif
 #else
 #define PROBE(p, bit) false
 #define TRACE(role, t, ev) do { } while (0)
 #define TRACE1(role, t, ev) do { } while (0)
+#define TRACED(role, t, ev) do { } while (0)
 #endif
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------
@@ -362,11 +368,28 @@ __device__ __forceinline__ float max33(float m, const float* x) {
     return max3(b, c, d);
 }
 
+constexpr uint32_t NONE = 0xffffffffu;
 struct EpiState {
     float m;       // running max of this row over the current document's tokens seen so far
     uint32_t k;    // documents of the current tile already finished
     uint32_t np;   // documents parked in the warp's buffer
+    // Two epilogue warp sets on alternate tiles: a tile is reduced before the running max of the previous tile (the
+    // other set's) is known.  Until that carry has been folded in (`unresolved`), the first document the tile closes is
+    // parked without it: `first` is its slot in the park buffer (NONE: nothing closed yet), `head` the value parked.
+    bool unresolved;
+    uint32_t first;
+    float head;
 };
+// a document closes with row maximum `value`
+__device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pend, uint32_t doc, int lane) {
+    if (s.unresolved && s.first == NONE) {
+        s.first = s.np;
+        s.head = value;
+    }
+    park(value, s.k, s.np, pend, doc, lane);
+    ++s.k;
+    ++s.np;
+}
 
 // 8 accumulator columns in which documents end (bit c of `byte`: column c is a document's last token): columns
 // are folded in order and every finished document is parked.  Out of line: boundary chunks are the minority, and
@@ -391,8 +414,10 @@ __device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float
 // 32 accumulator columns (registers v) with boundary word w: bit c set = column c is a document's last token.
 // Words without a boundary (the majority) take sixteen 3-input max instructions, and so does a word whose only
 // boundary is its last column (uniform 128-token documents).  Otherwise the word is walked in 8-column chunks.
+// `resolve` folds the previous tile's carry in; it must have run before the park buffer is drained.
+template <class Resolve>
 __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, uint32_t pend, uint32_t doc, float* out, int64_t B, uint32_t cfg, int lane,
-                                          bool skip_math) {
+                                          bool skip_math, Resolve resolve) {
     if (skip_math) {  // measurement probe: TMEM loads without the reduction
         s.m = fmaxf(s.m, v[0]);
         return;
@@ -403,12 +428,11 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
     }
     if (w == 0x80000000u) {
         if (s.np == PEND) {
+            if (s.unresolved) resolve();
             drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
-        park(max33(s.m, v), s.k, s.np, pend, doc, lane);
-        ++s.k;
-        ++s.np;
+        close_doc(max33(s.m, v), s, pend, doc, lane);
         s.m = -INFINITY;
         return;
     }
@@ -421,6 +445,7 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
             continue;
         }
         if (s.np + __popc(byte) > PEND) {  // room for the documents that end in this chunk
+            if (s.unresolved) resolve();
             drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
@@ -435,12 +460,15 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
                 l[c] = left ? x[c] : -INFINITY;
                 r[c] = left ? -INFINITY : x[c];
             }
-            park(max9(s.m, l), s.k, s.np, pend, doc, lane);
+            close_doc(max9(s.m, l), s, pend, doc, lane);
             s.m = max9(-INFINITY, r);  // Alg. 3 line 4 for the next document, then its first columns
-            ++s.k;
-            ++s.np;
         } else {
+            const bool rec = s.unresolved && s.first == NONE;
             s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.k, s.np, pend, doc, lane);
+            if (rec) {  // the first document this tile closes was parked by the helper: pick its value up again
+                s.first = s.np;
+                s.head = lds_f32(pend + (s.np * PEND_PITCH + lane) * 4);
+            }
             const uint32_t n = __popc(byte);
             s.k += n;
             s.np += n;
@@ -460,8 +488,10 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
 // split them into bf16 hi/lo and write the same operand stages as the fp32 path.  The decompressed vectors exist only
 // as MMA operands in shared memory, never in HBM (P:L244-249 names decompress-then-score as the costly baseline
 // because of its HBM round trip; on-chip it costs 16 bytes of HBM per token and no lookup per query row).
-template <int MB, int KBS, bool F32, bool PQD>
-__global__ void __launch_bounds__(128 + 128 * MB + (F32 ? 128 : 0), 1)
+// NSET: epilogue warp sets.  2 (16-bit inputs only): two warps per 32 TMEM lanes, one per half of a tile's columns --
+// pays when documents are short (many boundaries per tile: the segmented reduction is the binding step); 1 otherwise.
+template <int MB, int KBS, bool F32, bool PQD, int NSET>
+__global__ void __launch_bounds__(128 + NSET * 128 * MB + (F32 ? 128 : 0), 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
@@ -470,13 +500,15 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     constexpr uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
     constexpr uint32_t raw_bytes = PQD ? BN * 16u : 2u * KB_TILE_BYTES;  // PQD: 16 code bytes per token
     constexpr uint32_t cb_bytes = PQD ? 16u * 256u * 8u * 4u : 0u;        // PQD: the codebook [16][256][8], as two bf16 planes
-    constexpr int n_epi_warps = 4 * MB;
+    constexpr int n_epi_warps = 4 * MB;            // epilogue warps of one set (one set reduces a tile)
+    static_assert(NSET == 1 || (NSET == 2 && !F32), "two epilogue sets exist for 16-bit inputs only");
     uint8_t* st_ptr = smem;
     uint8_t* rw_ptr = st_ptr + (size_t)p.NS * stage_bytes;
     uint8_t* cb_ptr = rw_ptr + (F32 ? (size_t)p.NR * raw_bytes : 0);
     SegInfo* seg = reinterpret_cast<SegInfo*>(cb_ptr + cb_bytes);
     float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps]{[PEND][PEND_PITCH] maxima, [PEND] ids}
-    uint64_t* bars = reinterpret_cast<uint64_t*>(pend_all + n_epi_warps * PEND * (PEND_PITCH + 1));
+    float* mail = pend_all + NSET * n_epi_warps * PEND * (PEND_PITCH + 1);         // [NSET][warps][32] carries between the sets
+    uint64_t* bars = reinterpret_cast<uint64_t*>(mail + 2 * 8 * 32);
     uint64_t* full = bars;                       // [NS]   operand stage filled (TMA, or the splitter warps) -> MMA
     uint64_t* empty = full + MAX_STAGES;         // [NS]   operand stage read by the tensor pipe -> TMA / splitter
     uint64_t* tfull = empty + MAX_STAGES;        // [4*MB] MMA -> epilogue: accumulator of (tile t, block mb), ring t & 3
@@ -487,8 +519,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint64_t* rempty = rfull + MAX_RAW;          // [NR]   F32: splitter -> TMA (4 warps)
     uint64_t* aready = rempty + MAX_RAW;         // [1]    query rows are in TMEM
     uint64_t* turn = aready + 1;                 // [2]    MMA issuer w may start its next tile (the other one is done issuing)
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(turn + 2);
-    int64_t* range = reinterpret_cast<int64_t*>(turn + 3);  // b_lo, b_hi, t_lo, t_hi
+    uint64_t* carry = turn + 2;                  // [2][8] epilogue set -> the other set: running maxima at the end of a tile
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(carry + 16);
+    int64_t* range = reinterpret_cast<int64_t*>(carry + 17);  // b_lo, b_hi, t_lo, t_hi
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -497,12 +530,13 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         if (lane == 0) {
             for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), F32 ? 4 : 1); mbar_init(smem_u32(empty + s), 1); }
             for (int s = 0; s < 8; ++s) mbar_init(smem_u32(tfull + s), 1);
-            for (int s = 0; s < MAX_ACC; ++s) mbar_init(smem_u32(tempty + s), 4);
+            for (int s = 0; s < MAX_ACC; ++s) mbar_init(smem_u32(tempty + s), 4 * NSET);
             for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
-            for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), n_epi_warps); }
+            for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), NSET * n_epi_warps); }
             mbar_init(smem_u32(aready), n_epi_warps);
             mbar_init(smem_u32(turn), 1);
             mbar_init(smem_u32(turn + 1), 1);
+            for (int s = 0; s < 16; ++s) mbar_init(smem_u32(carry + s), 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
             if (!PQD) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
         }
@@ -564,7 +598,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     }
                 } else {
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
-                    if (ch == 0) TRACE(0, t, 0);
+                    if (ch == 0) TRACED(0, t, 0);
 #ifdef TMS_PROBES
                     if (PROBE(p, 8)) {  // probe: one linear 1-D bulk copy per stage instead of the 2-D tensor copies (wrong data layout, timing only)
                         if (elect_one()) {
@@ -582,7 +616,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     }
                 }
                 __syncwarp();
-                if (ch == nchunks - 1) TRACE(0, t, 2);
+                if (ch == nchunks - 1) TRACED(0, t, 2);
                 if (++s == nring) { s = 0; ph ^= 1; }
             }
         }
@@ -601,53 +635,59 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t w = (uint32_t)warp >> 1;  // 0: even tiles, 1: odd tiles
         mbar_wait(smem_u32(aready), 0);
         tc_fence_after();
+        // Everything below is computed by the whole warp (warp-uniform values stay in the uniform datapath, where a
+        // descriptor is the previous one plus a constant); only the tcgen05 instructions sit in elect_one() regions.
         const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
         const uint32_t idesc = p.idesc;
         const bool skip = PROBE(p, 2), skip_alo = p.skip_alo != 0;
-        const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS;
+        const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS, nch = (uint32_t)nchunks;
         const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
         // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
         const uint32_t a_lo_off = (uint32_t)p.NKB * KB_WORDS;
         const uint32_t a_mb_step = F32 ? 2 * a_lo_off : a_lo_off;
         const bool epi_frees_stage = !F32 && nchunks == 1;
-        const uint32_t full0 = smem_u32(full), tempty0 = smem_u32(tempty), tfull0 = smem_u32(tfull);
+        const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), tempty0 = smem_u32(tempty), tfull0 = smem_u32(tfull);
         const uint32_t my_turn = smem_u32(turn + w), other_turn = smem_u32(turn + (w ^ 1));
         // ring positions of this warp's first tile (tile w): operand stage w*nchunks, accumulator jobs w*MB + mb
-        uint32_t s = 0, ph = 0;
-        for (uint32_t c = 0; c < w * (uint32_t)nchunks; ++c)
-            if (++s == NS) { s = 0; ph ^= 1; }
+        uint32_t s = w * nch, ph = 0;
+        while (s >= NS) { s -= NS; ph ^= 1; }
         uint32_t slot[MB], tph[MB];
 #pragma unroll
         for (int mb = 0; mb < MB; ++mb) {
-            slot[mb] = 0; tph[mb] = 0;
-            for (uint32_t c = 0; c < w * MB + (uint32_t)mb; ++c)
-                if (++slot[mb] == nacc) { slot[mb] = 0; tph[mb] ^= 1; }
+            slot[mb] = w * MB + mb; tph[mb] = 0;
+            while (slot[mb] >= nacc) { slot[mb] -= nacc; tph[mb] ^= 1; }
         }
-        const bool early_full = NS > (uint32_t)nchunks, early_acc = nacc > (uint32_t)MB;
-        uint32_t tp = 0;  // parity of `turn` to wait for; warp 1's first tile (tile 0) needs no hand-over
-        for (int64_t t = w; t < ntiles; t += 2) {
-            // The tile's first stage and first accumulator are awaited BEFORE the hand-over when that is safe: a
-            // parity wait is only meaningful once the barrier's previous phase has completed, which is certain when
-            // that phase belongs to a tile <= t-2 (issued before this warp's previous hand-over), i.e. when the ring
-            // is longer than one tile's worth (NS > nchunks, NACC > MB).  Otherwise they are awaited after it.
+        // The tile's first stage and first accumulator are awaited BEFORE the hand-over when that is safe: a parity
+        // wait is only meaningful once the barrier's previous phase has completed, which is certain when that phase
+        // belongs to a tile <= t-2 (issued before this warp's previous hand-over), i.e. when the ring is longer
+        // than one tile's worth (NS > nchunks, NACC > MB).  Otherwise they are awaited after it.
+        const bool early_full = NS > nch, early_acc = nacc > (uint32_t)MB;
+        uint32_t tp = 0;             // parity of `turn` to wait for; tile 0 needs no hand-over
+        uint32_t tq = w;             // t & 3 of this warp's tile: the tfull ring
+        const int nt = (int)ntiles;
+        for (int t = (int)w; t < nt; t += 2) {
             if (early_full) mbar_wait(full0 + s * 8, ph);
             if (early_acc) mbar_wait(tempty0 + slot[0] * 8, tph[0] ^ 1);  // the epilogue has drained block 0's accumulator
             if (t != 0) { mbar_wait(my_turn, tp); tp ^= 1; }
-            if (!early_full) mbar_wait(full0 + s * 8, ph);
-            if (!early_acc) mbar_wait(tempty0 + slot[0] * 8, tph[0] ^ 1);
-            tc_fence_after();
             TRACE(1, t, 0);
-            if (elect_one()) {
-                uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
-                uint32_t sc = s, phc = ph;
-                for (int ch = 0; ch < nchunks; ++ch) {
-                    if (ch != 0) { mbar_wait(full0 + sc * 8, phc); tc_fence_after(); }
-                    const uint32_t b_lo = b_lo0 + sc * (stage_bytes >> 4);
-                    const bool last_chunk = ch == nchunks - 1;
+#ifdef TMS_PROBES
+            if (blockIdx.x == TRACE_CTA && lane == 0 && t >= TRACE_T0 && t < TRACE_T0 + TRACE_NT) {
+                uint64_t gt;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+                g_trace[(1 * TRACE_NT + (int)(t - TRACE_T0)) * TRACE_EV + 7] = (long long)gt;
+            }
+#endif
+            uint32_t a_col = tmem_base;  // this chunk's first dimension block of query block 0
+            for (uint32_t ch = 0; ch < nch; ++ch) {
+                if (ch != 0 || !early_full) mbar_wait(full0 + s * 8, ph);
+                const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
+                const bool last_chunk = ch == nch - 1;
 #pragma unroll
-                    for (int mb = 0; mb < MB; ++mb) {
-                        if (ch == 0 && mb != 0) { mbar_wait(tempty0 + slot[mb] * 8, tph[mb] ^ 1); tc_fence_after(); }
-                        const uint32_t d_tmem = acc0 + slot[mb] * BN;
+                for (int mb = 0; mb < MB; ++mb) {
+                    if (ch == 0 && !(mb == 0 && early_acc)) mbar_wait(tempty0 + slot[mb] * 8, tph[mb] ^ 1);
+                    tc_fence_after();
+                    const uint32_t d_tmem = acc0 + slot[mb] * BN;
+                    if (elect_one()) {
                         if (!skip) {
                             if constexpr (F32) {
 #pragma unroll
@@ -678,24 +718,25 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         // accumulator -> epilogue.  When a tile is a single stage, the last block's barrier also tells
                         // the epilogue that the stage has been read (it hands the stage back to the producer): one
                         // tcgen05.commit fewer per tile.
-                        if (last_chunk) tc_commit(tfull0 + ((uint32_t)(t & 3) * MB + mb) * 8);
-                        if (mb == MB - 1 && !epi_frees_stage) tc_commit(smem_u32(empty + sc));
+                        if (last_chunk) tc_commit(tfull0 + (tq * MB + mb) * 8);
+                        if (mb == MB - 1 && !epi_frees_stage) tc_commit(empty0 + s * 8);
                         if (last_chunk && mb == MB - 1) mbar_arrive(other_turn);  // the other issuer may start its tile
                     }
-                    a_col += (F32 ? 1 : KBS) * KB_WORDS;
-                    if (++sc == NS) { sc = 0; phc ^= 1; }
+                    __syncwarp();
                 }
-            }
-            __syncwarp();
-            TRACE(1, t, 4);
-            // this warp's next tile is two tiles on
-            for (int c = 0; c < 2 * nchunks; ++c)
+                a_col += (F32 ? 1 : KBS) * KB_WORDS;
                 if (++s == NS) { s = 0; ph ^= 1; }
+            }
+            TRACED(1, t, 4);
+            // this warp's next tile is two tiles on: skip the other warp's stages and accumulators
+            s += nch;
+            while (s >= NS) { s -= NS; ph ^= 1; }
 #pragma unroll
             for (int mb = 0; mb < MB; ++mb) {
                 slot[mb] += 2 * MB;
                 while (slot[mb] >= nacc) { slot[mb] -= nacc; tph[mb] ^= 1; }
             }
+            tq ^= 2;
         }
     } else if (warp == 2) {
         // ===== document segmenter =====
@@ -756,11 +797,11 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // documents after the last token of the range can only be empty
         for (int64_t idx = wb + consumed + lane; idx < b_hi; idx += 32)
             for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
-    } else if (F32 && warp >= 4 + n_epi_warps) {
+    } else if (F32 && warp >= 4 + NSET * n_epi_warps) {
         // ===== fp32 splitter (F32 only): raw fp32 stage -> bf16 hi block + bf16 lo block of an operand stage =====
         // Thread r owns token row r of the tile.  Both layouts are the 128-byte swizzle (16-byte piece index XOR
         // row % 8), so the eight rows a quarter-warp touches in one instruction fall into eight different bank groups.
-        const int r = threadIdx.x - 32 * (4 + n_epi_warps);
+        const int r = threadIdx.x - 32 * (4 + NSET * n_epi_warps);
         const uint32_t sw = (uint32_t)(r & 7);
         uint32_t s = 0, ph = 0, rs = 0, rph = 0;
         const int64_t nunits = ntiles * nchunks;
@@ -841,14 +882,16 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         }
     } else if (warp >= 4) {
         // ===== epilogue: running rowmax, segmented by document; max -> sum =====
-        const int ew = warp - 4, mb = ew >> 2, quad = warp & 3;
+        const int set = (warp - 4) / n_epi_warps;            // which half of every tile's columns is this warp's (NSET == 2)
+        const int ew = (warp - 4) % n_epi_warps, mb = ew >> 2, quad = warp & 3;
         const int row = mb * 128 + quad * 32 + lane;   // this thread's query row = TMEM lane quad*32+lane of block mb
         const int q = row / p.Nq_pad, i = row - q * p.Nq_pad;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quad * 32) << 16);
 
         // a2: the thread's query row -> TMEM, two 16-bit elements per column: columns [mb*NKB*32, +NKB*32), or for
         // F32 the bf16 hi halves in [mb*2*NKB*32, +NKB*32) followed by the lo halves.  Rows no query token owns
-        // are zero (finite similarities that never reach a score, A5).
+        // are zero (finite similarities that never reach a score, A5).  Done by the first set only.
+        if (set == 0)
         {
             const bool row_valid = (q < p.Q) && (i < p.Nq);
             const uint8_t* src = static_cast<const uint8_t*>(p.queries) + ((int64_t)q * p.Nq + i) * p.row_bytes;
@@ -913,38 +956,56 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const int nvalid = p.Q - q0 < 0 ? 0 : (p.Q - q0 < nsub ? p.Q - q0 : nsub);
         const uint32_t cfg = pack_cfg(p.Nq, p.Nq_pad, nvalid);
         float* out = p.scores + (int64_t)q0 * p.B + b_lo;
-        const uint32_t pend = smem_u32(pend_all) + (uint32_t)ew * (PEND_IDS + PEND * 4);
+        const uint32_t pend = smem_u32(pend_all) + (uint32_t)(warp - 4) * (PEND_IDS + PEND * 4);
         const bool skip_math = PROBE(p, 1);
         const int64_t B = p.B;
-        const bool frees_stage = !F32 && nchunks == 1 && ew == 4 * (MB - 1);  // see the MMA warp
+        const bool frees_stage = !F32 && nchunks == 1 && set == 0 && ew == 4 * (MB - 1);  // see the MMA warps
+
+        // Two sets (16-bit inputs): set 0 reduces columns 0..63 of every tile, set 1 columns 64..127.  A tcgen05.ld
+        // blocks the issuing warp until its data are in registers (measured: two loads "in flight" from one warp take
+        // as long as two in sequence, ~90 clk per 32 columns), so a warp cannot overlap its own TMEM reads with its
+        // own arithmetic; a second warp on the same sub-partition and TMEM lanes can, and the accumulator goes back to
+        // the MMA warps after two loads per warp instead of four.  The running maximum crosses a range boundary through a
+        // 32-float mailbox: a range is reduced from -inf, the first document it closes is parked provisionally, and only
+        // at the END of the range is the previous range's carry awaited and folded in (into that parked value, or into
+        // the still open segment), after which the range's own carry goes to the other set.  The serial chain per
+        // tile is therefore two mailbox hops, not two range reductions.
+        const uint32_t mail_out = smem_u32(mail) + (uint32_t)((set * 8 + ew) * 32 + lane) * 4;
+        const uint32_t mail_in = smem_u32(mail) + (uint32_t)(((set ^ 1) * 8 + ew) * 32 + lane) * 4;
+        const uint32_t carry_out = smem_u32(carry + set * 8 + ew), carry_in = smem_u32(carry + (set ^ 1) * 8 + ew);
+        uint32_t cph = 0;
 
         EpiState st;
         st.m = -INFINITY;  // Alg. 3 line 4
         st.k = 0;
         st.np = 0;
-        const uint32_t nacc = (uint32_t)p.NACC;
+        st.unresolved = false;
+        st.first = NONE;
+        st.head = 0.f;
+        auto resolve = [&]() {
+            if constexpr (NSET == 2) {
+                mbar_wait(carry_in, cph);
+                cph ^= 1;
+                const float cin = lds_f32(mail_in);
+                if (st.first != NONE) sts_f32(pend + (st.first * PEND_PITCH + lane) * 4, fmaxf(st.head, cin));
+                else st.m = fmaxf(st.m, cin);  // nothing closed yet: the open segment continues the previous tile's
+                st.unresolved = false;
+            }
+        };
+        const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS;
         const uint32_t acc0 = lane_addr + (uint32_t)p.acc_col0;
-        uint32_t slot = (uint32_t)mb, tph = 0, g = 0, gph = 0, rs = 0;
+        uint32_t slot = (uint32_t)mb, g = 0, gph = 0, rs = 0;
+        const bool tr = quad == 0 && set == 0;  // (probe builds) the warp whose clock is traced
         for (int64_t t = 0; t < ntiles; ++t) {
-            if (quad == 0) TRACE(2 + mb, t, 0);
+            if (tr) TRACED(2 + mb, t, 0);
             mbar_wait(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb), (uint32_t)(t >> 2) & 1u);
             tc_fence_after();
-            if (quad == 0) TRACE(2 + mb, t, 1);
             if (frees_stage) {  // the tile's only stage has been read by the tensor pipe: back to the producer
                 if (lane == 0) mbar_arrive(smem_u32(empty + rs));
-                if (++rs == (uint32_t)p.NS) rs = 0;
+                if (++rs == NS) rs = 0;
             }
+            if (tr) TRACED(2 + mb, t, 1);
             const uint32_t taddr = acc0 + slot * BN;
-            if (PROBE(p, 4)) {  // measurement probe: no TMEM reads at all
-                mbar_wait(smem_u32(sfull + g), gph);
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) { mbar_arrive(smem_u32(tempty + slot)); mbar_arrive(smem_u32(sempty + g)); }
-                slot += MB;
-                if (slot >= nacc) { slot -= nacc; tph ^= 1; }
-                if (++g == NSEG) { g = 0; gph ^= 1; }
-                continue;
-            }
             if constexpr (F32) {
                 // 512 threads leave 128 registers each: the accumulator is read in two halves of 64 columns.  A tile
                 // costs the tensor pipe three MMAs per K step here, so the later release is off the critical path.
@@ -957,8 +1018,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 st.k = 0;
                 tmem_ld_wait32(v);
                 tmem_ld_pin32(v + 32);
-                process32(v, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
-                process32(v + 32, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
+                process32(v, mask.x, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
+                process32(v + 32, mask.y, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
                 tmem_ld32(taddr + 64, v);
                 tmem_ld32(taddr + 96, v + 32);
                 tmem_ld_wait32(v);
@@ -966,65 +1027,49 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-                process32(v, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
-                process32(v + 32, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
-            } else if constexpr (MB == 2) {
-                // Two epilogue warps share each scheduler: 32 columns at a time, the next load in flight while the current columns are reduced (a TMEM load of
-                // 32 columns x 32 lanes occupies the warp's TMEM port for about as long as reducing them takes); the
-                // accumulator goes back to the MMA warp as soon as its last column is in registers.
-                float va[32], vb[32];
-                tmem_ld32(taddr, va);
-                mbar_wait(smem_u32(sfull + g), gph);
-                const uint32_t doc = smem_u32(seg[g].doc);
-                const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
-                st.k = 0;
-                tmem_ld_wait32(va);
-                if (quad == 0) TRACE(2 + mb, t, 2);
-                tmem_ld32(taddr + 32, vb);
-                process32(va, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
-                tmem_ld_wait32(vb);
-                if (quad == 0) TRACE(2 + mb, t, 3);
-                tmem_ld32(taddr + 64, va);
-                process32(vb, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
-                tmem_ld_wait32(va);
-                if (quad == 0) TRACE(2 + mb, t, 4);
-                tmem_ld32(taddr + 96, vb);
-                process32(va, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
-                tmem_ld_wait32(vb);
-                if (quad == 0) TRACE(2 + mb, t, 5);
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-                process32(vb, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
-                if (quad == 0) TRACE(2 + mb, t, 6);
+                process32(v, mask.z, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
+                process32(v + 32, mask.w, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
             } else {
-                // One epilogue warp per scheduler: every extra tcgen05.wait::ld costs more than the overlap gains, so the
-                // whole accumulator is loaded at once and handed back to the MMA warp before any of it is reduced.
-                float v[BN];
-                tmem_ld32(taddr, v);
-                tmem_ld32(taddr + 32, v + 32);
-                tmem_ld32(taddr + 64, v + 64);
-                tmem_ld32(taddr + 96, v + 96);
+                float v[32];
+                constexpr int NW = 4 / NSET;                   // 32-column words of a tile that are this warp's
+                const uint32_t c0 = (uint32_t)set * (NW * 32);  // its first column
+                tmem_ld32(taddr + c0, v);
                 mbar_wait(smem_u32(sfull + g), gph);
                 const uint32_t doc = smem_u32(seg[g].doc);
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
-                st.k = 0;
-                tmem_ld_wait32(v);
-                tmem_ld_pin32(v + 32);
-                tmem_ld_pin32(v + 64);
-                tmem_ld_pin32(v + 96);
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-                process32(v, mask.x, st, pend, doc, out, B, cfg, lane, skip_math);
-                process32(v + 32, mask.y, st, pend, doc, out, B, cfg, lane, skip_math);
-                process32(v + 64, mask.z, st, pend, doc, out, B, cfg, lane, skip_math);
-                process32(v + 96, mask.w, st, pend, doc, out, B, cfg, lane, skip_math);
+                const uint32_t wds[4] = {mask.x, mask.y, mask.z, mask.w};
+                st.k = (NSET == 2 && set) ? __popc(mask.x) + __popc(mask.y) : 0;
+                if (NSET == 2 && (set != 0 || t != 0)) {  // reduced from -inf; the previous range's carry is folded in at the end
+                    st.m = -INFINITY;
+                    st.unresolved = true;
+                    st.first = NONE;
+                }
+#pragma unroll
+                for (int i = 0; i < NW; ++i) {
+                    if (i) tmem_ld32(taddr + c0 + 32 * i, v);
+                    tmem_ld_wait32(v);
+                    if (i == NW - 1) {  // this warp's columns are in registers
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
+                    }
+                    if (tr) TRACED(2 + mb, t, 2 + i);
+                    process32(v, wds[(NSET == 2 && set ? 2 : 0) + i], st, pend, doc, out, B, cfg, lane, skip_math, resolve);
+                }
+                if constexpr (NSET == 2) {
+                    if (st.unresolved) resolve();
+                    if (set == 0 || t + 1 < ntiles) {  // this range's carry -> the other set
+                        sts_f32(mail_out, st.m);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(carry_out);
+                    }
+                }
+                if (tr) TRACED(2 + mb, t, 6);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
             slot += MB;
-            if (slot >= nacc) { slot -= nacc; tph ^= 1; }
+            if (slot >= nacc) slot -= nacc;
             if (++g == NSEG) { g = 0; gph ^= 1; }
         }
         if (st.np) drain(pend, st.np, out, B, cfg, lane);
@@ -1105,13 +1150,14 @@ struct Plan {
     bool pqd;           // decode-and-contract PQ variant
     int nparts;         // equal parts a query is scored in (1 unless Nq > 32)
     int Qg;             // queries per launch
+    int nset;           // epilogue warp sets
     uint32_t smem_bytes;
 };
 
-uint32_t fixed_smem(int MB) {
-    const uint32_t warps = 4u * MB;
+uint32_t fixed_smem(int MB, int nset) {
+    const uint32_t warps = (uint32_t)nset * 4u * MB;
     return (uint32_t)sizeof(SegInfo) * NSEG + warps * PEND * (PEND_PITCH + 1) * 4 +
-           8u * (2 * MAX_STAGES + 8 + MAX_ACC + 2 * NSEG + 2 * MAX_RAW + 4) + 4 * 8 + 1024 /* alignment slack */;
+           2 * 8 * 32 * 4 + 8u * (2 * MAX_STAGES + 8 + MAX_ACC + 2 * NSEG + 2 * MAX_RAW + 4 + 16) + 4 * 8 + 1024 /* alignment slack */;
 }
 
 // Shape -> kernel parameters; false when the tcgen05 path does not cover it.
@@ -1172,8 +1218,14 @@ bool plan(const DenseArgs& a, Plan& pl) {
     pl.nparts = nparts;
     pl.f32 = f32;
     pl.pqd = pqd;
+    // two epilogue sets when documents are short on average (< 100 tokens: most tiles then hold a document boundary
+    // or several, and the segmented reduction binds), measured on config 3 (mean 72 tokens) against config 2 (128)
+    pl.nset = (!f32 && a.T < 100 * a.B) ? 2 : 1;
+#ifdef TMS_PROBES
+    if (const char* e = getenv("TMS_NSET")) { const int n = atoi(e); if (!f32 && (n == 1 || n == 2)) pl.nset = n; }
+#endif
     pl.KBS = f32 ? 2 : ((NKB % 2 == 0) ? 2 : 1);
-    const uint32_t fixed = fixed_smem(MB);
+    const uint32_t fixed = fixed_smem(MB, pl.nset);
     const uint32_t stage_bytes = (uint32_t)pl.KBS * KB_TILE_BYTES;
     int ns = (int)((SMEM_LIMIT - fixed) / stage_bytes);
     p.NR = 0;
@@ -1230,10 +1282,15 @@ int launch_dense_tc(const DenseArgs& a) {
         return TMS_ERR_CUDA;
 
     void (*kern)(const CUtensorMap, const Params) = nullptr;
-    if (pl.pqd) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, true> : dense_tc_kernel<2, 2, true, true>;
-    else if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, false> : dense_tc_kernel<2, 2, true, false>;
-    else if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false> : dense_tc_kernel<1, 2, false, false>;
-    else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false> : dense_tc_kernel<2, 2, false, false>;
+    if (pl.pqd) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, true, 1> : dense_tc_kernel<2, 2, true, true, 1>;
+    else if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, false, 1> : dense_tc_kernel<2, 2, true, false, 1>;
+    else if (pl.nset == 1) {
+        if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 1> : dense_tc_kernel<1, 2, false, false, 1>;
+        else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 1> : dense_tc_kernel<2, 2, false, false, 1>;
+    } else {
+        if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 2> : dense_tc_kernel<1, 2, false, false, 2>;
+        else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 2> : dense_tc_kernel<2, 2, false, false, 2>;
+    }
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess)
         return TMS_ERR_CUDA;
     // no more CTAs than 128-token tiles; one CTA per SM
@@ -1251,7 +1308,7 @@ int launch_dense_tc(const DenseArgs& a) {
         p.Q = Qeff - q0 < pl.Qg ? Qeff - q0 : pl.Qg;
         p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * p.Nq * p.row_bytes;
         p.scores = dst + (int64_t)q0 * a.B;
-        kern<<<(unsigned)grid, 128 + 128 * pl.MB + (pl.f32 ? 128 : 0), pl.smem_bytes, a.stream>>>(map_docs, p);
+        kern<<<(unsigned)grid, 128 + pl.nset * 128 * pl.MB + (pl.f32 ? 128 : 0), pl.smem_bytes, a.stream>>>(map_docs, p);
         count_launch();
         if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
     }
