@@ -116,6 +116,8 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// The suspend-time hint lets the hardware park the warp until the phase completes (or the hint expires) instead of
+// returning early: a warp that spins on try_wait takes issue slots from the working warps of its sub-partition.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
@@ -126,7 +128,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "bra LAB_WAIT;\n"
         "DONE:\n"
         "}\n" ::"r"(bar),
-        "r"(parity)
+        "r"(parity), "r"(0x989680u)
         : "memory");
 }
 // non-blocking: has the phase with this parity completed?
@@ -278,9 +280,11 @@ __device__ int64_t warp_lower_bound(const int64_t* __restrict__ offsets, int64_t
 
 struct SegInfo {
     uint32_t mask[4];     // bit c set: column c of the tile is the last token of a (non-empty) document
-    uint32_t pad[4];
-    uint32_t doc[BN];     // k-th set bit  ->  document index relative to the CTA's first document
 };
+// The CTA's non-empty documents are numbered in order ("ordinals"); DOCRING maps ordinal -> document index relative to
+// the CTA's first document.  The segmenter is at most NSEG tiles (<= 128 documents each) ahead of the slowest epilogue
+// warp, which holds at most PEND parked documents plus its current tile's: 16 + 128 + 512 < DOCRING entries are live.
+constexpr uint32_t DOCRING = 1024;
 
 // ---- epilogue helpers ------------------------------------------------------------------------------------------
 __device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }  // one FMNMX3
@@ -318,12 +322,11 @@ __device__ __forceinline__ float lds_f32(uint32_t addr) {
 }
 
 // A document's last token has been folded in: row `lane` parks its maximum in slot np of the warp's buffer.
-// pend: shared-window byte address of this warp's park buffer ([PEND][PEND_PITCH] floats, then PEND document ids);
-// doc: shared-window byte address of the current tile's list of ending documents.
+// pend: shared-window byte address of this warp's park buffer ([PEND][PEND_PITCH] floats, then PEND document ordinals).
 constexpr uint32_t PEND_IDS = PEND * PEND_PITCH * 4;  // byte offset of the ids inside a warp's park buffer
-__device__ __forceinline__ void park(float m, uint32_t k, uint32_t np, uint32_t pend, uint32_t doc, int lane) {
+__device__ __forceinline__ void park(float m, uint32_t ord, uint32_t np, uint32_t pend, int lane) {
     sts_f32(pend + (np * PEND_PITCH + lane) * 4, m);
-    if (lane == 0) sts_u32(pend + PEND_IDS + np * 4, lds_u32(doc + k * 4));
+    if (lane == 0) sts_u32(pend + PEND_IDS + np * 4, ord);
 }
 
 // max -> sum (Eq. 1) for the np parked documents.  Rows that no query token owns hold zero query vectors, so their
@@ -332,7 +335,7 @@ __device__ __forceinline__ void park(float m, uint32_t k, uint32_t np, uint32_t 
 //   Nq_pad = 32 (one query per warp): lanes j and j+16 add rows 0..15 / 16..31 of parked document j with four
 //   16-byte loads each, in four interleaved partial sums, and lane j stores the score.
 //   Nq_pad < 32: one lane per (document, query of this warp), rows added in ascending order.
-__device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64_t B, uint32_t cfg, int lane) {
+__device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64_t B, uint32_t cfg, uint32_t ring, int lane) {
     const uint32_t Nq_pad = (cfg >> 6) & 63u, nvalid = (cfg >> 12) & 63u;
     __syncwarp();
     if (Nq_pad == 32) {
@@ -343,7 +346,7 @@ __device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64
         const float a2 = (x0.z + x1.z) + (x2.z + x3.z), a3 = (x0.w + x1.w) + (x2.w + x3.w);
         float acc = (a0 + a1) + (a2 + a3);
         acc += __shfl_xor_sync(0xffffffffu, acc, 16);
-        if (h == 0 && j < np && nvalid) out[lds_u32(pend + PEND_IDS + j * 4)] = acc;
+        if (h == 0 && j < np && nvalid) out[lds_u32(ring + (lds_u32(pend + PEND_IDS + j * 4) & (DOCRING - 1)) * 4)] = acc;
     } else {
         const uint32_t nsub = 32u / Nq_pad;
         for (uint32_t u = lane; u < np * nsub; u += 32) {
@@ -352,7 +355,7 @@ __device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64
                 const uint32_t p = pend + (slot * PEND_PITCH + sub * Nq_pad) * 4;
                 float acc = lds_f32(p);
                 for (uint32_t r = 1; r < Nq_pad; ++r) acc += lds_f32(p + r * 4);
-                out[(int64_t)sub * B + lds_u32(pend + PEND_IDS + slot * 4)] = acc;
+                out[(int64_t)sub * B + lds_u32(ring + (lds_u32(pend + PEND_IDS + slot * 4) & (DOCRING - 1)) * 4)] = acc;
             }
         }
     }
@@ -371,7 +374,7 @@ __device__ __forceinline__ float max33(float m, const float* x) {
 constexpr uint32_t NONE = 0xffffffffu;
 struct EpiState {
     float m;       // running max of this row over the current document's tokens seen so far
-    uint32_t k;    // documents of the current tile already finished
+    uint32_t ord;  // ordinal of the next document to close (see DOCRING)
     uint32_t np;   // documents parked in the warp's buffer
     // Two epilogue warp sets on alternate tiles: a tile is reduced before the running max of the previous tile (the
     // other set's) is known.  Until that carry has been folded in (`unresolved`), the first document the tile closes is
@@ -381,13 +384,13 @@ struct EpiState {
     float head;
 };
 // a document closes with row maximum `value`
-__device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pend, uint32_t doc, int lane) {
+__device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pend, int lane) {
     if (s.unresolved && s.first == NONE) {
         s.first = s.np;
         s.head = value;
     }
-    park(value, s.k, s.np, pend, doc, lane);
-    ++s.k;
+    park(value, s.ord, s.np, pend, lane);
+    ++s.ord;
     ++s.np;
 }
 
@@ -395,15 +398,15 @@ __device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pen
 // are folded in order and every finished document is parked.  Out of line: boundary chunks are the minority, and
 // one compact copy keeps the epilogue's hot loop short.  The caller has made sure the buffer has room.
 __device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float x3, float x4, float x5, float x6,
-                                             float x7, uint32_t byte, float m, uint32_t k, uint32_t np, uint32_t pend,
-                                             uint32_t doc, int lane) {
+                                             float x7, uint32_t byte, float m, uint32_t ord, uint32_t np, uint32_t pend,
+                                             int lane) {
     const float x[8] = {x0, x1, x2, x3, x4, x5, x6, x7};
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         m = fmaxf(m, x[c]);
         if (byte & (1u << c)) {
-            park(m, k, np, pend, doc, lane);
-            ++k;
+            park(m, ord, np, pend, lane);
+            ++ord;
             ++np;
             m = -INFINITY;  // Alg. 3 line 4 for the next document
         }
@@ -411,12 +414,43 @@ __device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float
     return m;
 }
 
+// max of 8 columns
+__device__ __forceinline__ float max8(const float* x) {
+    return max3(max3(x[0], x[1], x[2]), max3(x[3], x[4], x[5]), fmaxf(x[6], x[7]));
+}
+
+// One document ends in this word, at column e of chunk J (8-column chunks; J compile-time): the columns up to e close the
+// document (together with the running max m), the columns after e open the next one.  Whole chunks go to one side
+// unconditionally; only chunk J is split, branch-free, with selects.
+template <int J>
+__device__ __forceinline__ void split_word(const float* v, int e8, float m, float& closed, float& open) {
+    float l[8], r[8];
+    const float* x = v + 8 * J;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const bool left = e8 >= c;
+        l[c] = left ? x[c] : -INFINITY;
+        r[c] = left ? -INFINITY : x[c];
+    }
+    float a = max3(max8(l), m, -INFINITY), b = max8(r);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (i < J) a = fmaxf(a, max8(v + 8 * i));
+        if (i > J) b = fmaxf(b, max8(v + 8 * i));
+    }
+    closed = a;
+    open = b;
+}
+
 // 32 accumulator columns (registers v) with boundary word w: bit c set = column c is a document's last token.
-// Words without a boundary (the majority) take sixteen 3-input max instructions, and so does a word whose only
-// boundary is its last column (uniform 128-token documents).  Otherwise the word is walked in 8-column chunks.
-// `resolve` folds the previous tile's carry in; it must have run before the park buffer is drained.
+//   no boundary (the majority)              sixteen 3-input max instructions
+//   one boundary                            dispatched ONCE on the boundary's 8-column chunk (a lone warp pays ~15 clk per
+//                                           unpredicted branch, so no per-chunk tests), whole chunks folded to either side
+//                                           and the boundary chunk split with selects
+//   several boundaries (documents < 32 tokens)   walked in 8-column chunks
+// `resolve` folds the previous range's carry in; it must have run before the park buffer is drained.
 template <class Resolve>
-__device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, uint32_t pend, uint32_t doc, float* out, int64_t B, uint32_t cfg, int lane,
+__device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& s, uint32_t pend, uint32_t ring, float* out, int64_t B, uint32_t cfg, int lane,
                                           bool skip_math, Resolve resolve) {
     if (skip_math) {  // measurement probe: TMEM loads without the reduction
         s.m = fmaxf(s.m, v[0]);
@@ -426,14 +460,33 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
         s.m = max33(s.m, v);
         return;
     }
-    if (w == 0x80000000u) {
+    if (w == 0x80000000u) {  // the word's last column (uniform 128-token documents)
         if (s.np == PEND) {
             if (s.unresolved) resolve();
-            drain(pend, s.np, out, B, cfg, lane);
+            drain(pend, s.np, out, B, cfg, ring, lane);
             s.np = 0;
         }
-        close_doc(max33(s.m, v), s, pend, doc, lane);
-        s.m = -INFINITY;
+        close_doc(max33(s.m, v), s, pend, lane);
+        s.m = -INFINITY;  // Alg. 3 line 4 for the next document
+        return;
+    }
+    if ((w & (w - 1)) == 0) {
+        if (s.np == PEND) {
+            if (s.unresolved) resolve();
+            drain(pend, s.np, out, B, cfg, ring, lane);
+            s.np = 0;
+        }
+        float closed, open;
+        const int e = 31 - __clz((int)w), e8 = e & 7;
+        if (e < 16) {
+            if (e < 8) split_word<0>(v, e8, s.m, closed, open);
+            else split_word<1>(v, e8, s.m, closed, open);
+        } else {
+            if (e < 24) split_word<2>(v, e8, s.m, closed, open);
+            else split_word<3>(v, e8, s.m, closed, open);
+        }
+        close_doc(closed, s, pend, lane);
+        s.m = open;
         return;
     }
 #pragma unroll
@@ -446,33 +499,18 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
         }
         if (s.np + __popc(byte) > PEND) {  // room for the documents that end in this chunk
             if (s.unresolved) resolve();
-            drain(pend, s.np, out, B, cfg, lane);
+            drain(pend, s.np, out, B, cfg, ring, lane);
             s.np = 0;
         }
-        if ((byte & (byte - 1)) == 0) {
-            // exactly one document ends in this chunk, at column e: branch-free split into the columns up to e (they
-            // close the document) and the columns after e (they open the next one)
-            const int e = 31 - __clz((int)byte);
-            float l[8], r[8];
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const bool left = e >= c;
-                l[c] = left ? x[c] : -INFINITY;
-                r[c] = left ? -INFINITY : x[c];
-            }
-            close_doc(max9(s.m, l), s, pend, doc, lane);
-            s.m = max9(-INFINITY, r);  // Alg. 3 line 4 for the next document, then its first columns
-        } else {
-            const bool rec = s.unresolved && s.first == NONE;
-            s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.k, s.np, pend, doc, lane);
-            if (rec) {  // the first document this tile closes was parked by the helper: pick its value up again
-                s.first = s.np;
-                s.head = lds_f32(pend + (s.np * PEND_PITCH + lane) * 4);
-            }
-            const uint32_t n = __popc(byte);
-            s.k += n;
-            s.np += n;
+        const bool rec = s.unresolved && s.first == NONE;
+        s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.ord, s.np, pend, lane);
+        if (rec) {  // the first document this range closes was parked by the helper: pick its value up again
+            s.first = s.np;
+            s.head = lds_f32(pend + (s.np * PEND_PITCH + lane) * 4);
         }
+        const uint32_t n = __popc(byte);
+        s.ord += n;
+        s.np += n;
     }
 }
 
@@ -506,7 +544,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     uint8_t* rw_ptr = st_ptr + (size_t)p.NS * stage_bytes;
     uint8_t* cb_ptr = rw_ptr + (F32 ? (size_t)p.NR * raw_bytes : 0);
     SegInfo* seg = reinterpret_cast<SegInfo*>(cb_ptr + cb_bytes);
-    float* pend_all = reinterpret_cast<float*>(seg + NSEG);                         // [warps]{[PEND][PEND_PITCH] maxima, [PEND] ids}
+    uint32_t* docring = reinterpret_cast<uint32_t*>(seg + NSEG);                    // [DOCRING]
+    float* pend_all = reinterpret_cast<float*>(docring + DOCRING);                         // [warps]{[PEND][PEND_PITCH] maxima, [PEND] ids}
     float* mail = pend_all + NSET * n_epi_warps * PEND * (PEND_PITCH + 1);         // [NSET][warps][32] carries between the sets
     uint64_t* bars = reinterpret_cast<uint64_t*>(mail + 2 * 8 * 32);
     uint64_t* full = bars;                       // [NS]   operand stage filled (TMA, or the splitter warps) -> MMA
@@ -598,7 +637,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     }
                 } else {
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
-                    if (ch == 0) TRACED(0, t, 0);
+    
 #ifdef TMS_PROBES
                     if (PROBE(p, 8)) {  // probe: one linear 1-D bulk copy per stage instead of the 2-D tensor copies (wrong data layout, timing only)
                         if (elect_one()) {
@@ -616,7 +655,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     }
                 }
                 __syncwarp();
-                if (ch == nchunks - 1) TRACED(0, t, 2);
+
                 if (++s == nring) { s = 0; ph ^= 1; }
             }
         }
@@ -753,6 +792,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         int64_t e_cur = load_ends(wb), e_nxt = load_ends(wb + 32);
         int64_t s_first = t_lo;  // start of document wb
         int consumed = 0;        // documents of the current window already assigned to a tile
+        uint32_t ord = 0;        // non-empty documents of this CTA seen so far (DOCRING ordinals)
         for (int64_t t = 0; t < ntiles; ++t) {
             const uint32_t g = (uint32_t)(t % NSEG), gph = (uint32_t)((t / NSEG) & 1);
             const int64_t tile_start = t_lo + t * BN, tile_end = tile_start + BN;
@@ -770,7 +810,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 uint32_t w0 = 0, w1 = 0, w2 = 0, w3 = 0;
                 if (nonempty) {
                     const uint32_t col = (uint32_t)(e - 1 - tile_start);
-                    seg[g].doc[nseg + __popc(nb & lt_mask)] = (uint32_t)(idx - b_lo);
+                    docring[(ord + nseg + __popc(nb & lt_mask)) & (DOCRING - 1)] = (uint32_t)(idx - b_lo);
                     const uint32_t bit = 1u << (col & 31);
                     w0 = (col >> 5) == 0 ? bit : 0; w1 = (col >> 5) == 1 ? bit : 0;
                     w2 = (col >> 5) == 2 ? bit : 0; w3 = (col >> 5) == 3 ? bit : 0;
@@ -790,6 +830,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 e_nxt = load_ends(wb + 32);
                 consumed = 0;
             }
+            ord += nseg;
             if (lane == 0) { seg[g].mask[0] = m0; seg[g].mask[1] = m1; seg[g].mask[2] = m2; seg[g].mask[3] = m3; }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sfull + g));
@@ -882,7 +923,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         }
     } else if (warp >= 4) {
         // ===== epilogue: running rowmax, segmented by document; max -> sum =====
-        const int set = (warp - 4) / n_epi_warps;            // which half of every tile's columns is this warp's (NSET == 2)
+        int set = (warp - 4) / n_epi_warps;                  // which half of every tile's columns is this warp's (NSET == 2)
+        if (NSET == 2) asm volatile("" : "+r"(set));           // opaque: otherwise re-derived from %tid.x (S2R) at every use
         const int ew = (warp - 4) % n_epi_warps, mb = ew >> 2, quad = warp & 3;
         const int row = mb * 128 + quad * 32 + lane;   // this thread's query row = TMEM lane quad*32+lane of block mb
         const int q = row / p.Nq_pad, i = row - q * p.Nq_pad;
@@ -959,6 +1001,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t pend = smem_u32(pend_all) + (uint32_t)(warp - 4) * (PEND_IDS + PEND * 4);
         const bool skip_math = PROBE(p, 1);
         const int64_t B = p.B;
+        const uint32_t ring = smem_u32(docring);
         const bool frees_stage = !F32 && nchunks == 1 && set == 0 && ew == 4 * (MB - 1);  // see the MMA warps
 
         // Two sets (16-bit inputs): set 0 reduces columns 0..63 of every tile, set 1 columns 64..127.  A tcgen05.ld
@@ -977,7 +1020,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
 
         EpiState st;
         st.m = -INFINITY;  // Alg. 3 line 4
-        st.k = 0;
+        st.ord = 0;
         st.np = 0;
         st.unresolved = false;
         st.first = NONE;
@@ -995,16 +1038,19 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS;
         const uint32_t acc0 = lane_addr + (uint32_t)p.acc_col0;
         uint32_t slot = (uint32_t)mb, g = 0, gph = 0, rs = 0;
-        const bool tr = quad == 0 && set == 0;  // (probe builds) the warp whose clock is traced
-        for (int64_t t = 0; t < ntiles; ++t) {
-            if (tr) TRACED(2 + mb, t, 0);
+        uint32_t ord_tile = 0;  // (two sets) non-empty documents that ended in earlier tiles
+        const bool tr = quad == 0 && (set == 0 || mb == 0);  // (probe builds) the warps whose clocks are traced
+        const int trole = set == 0 ? 2 + mb : 0;
+        const int nt = (int)ntiles;
+        for (int t = 0; t < nt; ++t) {
+            if (tr) TRACED(trole, t, 0);
             mbar_wait(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb), (uint32_t)(t >> 2) & 1u);
             tc_fence_after();
             if (frees_stage) {  // the tile's only stage has been read by the tensor pipe: back to the producer
                 if (lane == 0) mbar_arrive(smem_u32(empty + rs));
                 if (++rs == NS) rs = 0;
             }
-            if (tr) TRACED(2 + mb, t, 1);
+            if (tr) TRACED(trole, t, 1);
             const uint32_t taddr = acc0 + slot * BN;
             if constexpr (F32) {
                 // 512 threads leave 128 registers each: the accumulator is read in two halves of 64 columns.  A tile
@@ -1013,13 +1059,11 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tmem_ld32(taddr, v);
                 tmem_ld32(taddr + 32, v + 32);
                 mbar_wait(smem_u32(sfull + g), gph);
-                const uint32_t doc = smem_u32(seg[g].doc);
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
-                st.k = 0;
                 tmem_ld_wait32(v);
                 tmem_ld_pin32(v + 32);
-                process32(v, mask.x, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
-                process32(v + 32, mask.y, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
+                process32(v, mask.x, st, pend, ring, out, B, cfg, lane, skip_math, resolve);
+                process32(v + 32, mask.y, st, pend, ring, out, B, cfg, lane, skip_math, resolve);
                 tmem_ld32(taddr + 64, v);
                 tmem_ld32(taddr + 96, v + 32);
                 tmem_ld_wait32(v);
@@ -1027,18 +1071,21 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
-                process32(v, mask.z, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
-                process32(v + 32, mask.w, st, pend, doc, out, B, cfg, lane, skip_math, resolve);
+                process32(v, mask.z, st, pend, ring, out, B, cfg, lane, skip_math, resolve);
+                process32(v + 32, mask.w, st, pend, ring, out, B, cfg, lane, skip_math, resolve);
             } else {
                 float v[32];
                 constexpr int NW = 4 / NSET;                   // 32-column words of a tile that are this warp's
                 const uint32_t c0 = (uint32_t)set * (NW * 32);  // its first column
                 tmem_ld32(taddr + c0, v);
                 mbar_wait(smem_u32(sfull + g), gph);
-                const uint32_t doc = smem_u32(seg[g].doc);
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
                 const uint32_t wds[4] = {mask.x, mask.y, mask.z, mask.w};
-                st.k = (NSET == 2 && set) ? __popc(mask.x) + __popc(mask.y) : 0;
+                if (NSET == 2) {  // ordinal of the first document that ends in this warp's columns
+                    const uint32_t lo = __popc(mask.x) + __popc(mask.y);
+                    st.ord = ord_tile + (set ? lo : 0);
+                    ord_tile += lo + __popc(mask.z) + __popc(mask.w);
+                }
                 if (NSET == 2 && (set != 0 || t != 0)) {  // reduced from -inf; the previous range's carry is folded in at the end
                     st.m = -INFINITY;
                     st.unresolved = true;
@@ -1053,18 +1100,18 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         __syncwarp();
                         if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
                     }
-                    if (tr) TRACED(2 + mb, t, 2 + i);
-                    process32(v, wds[(NSET == 2 && set ? 2 : 0) + i], st, pend, doc, out, B, cfg, lane, skip_math, resolve);
+                    if (tr) TRACED(trole, t, 2 + i);
+                    process32(v, wds[(NSET == 2 && set ? 2 : 0) + i], st, pend, ring, out, B, cfg, lane, skip_math, resolve);
                 }
                 if constexpr (NSET == 2) {
                     if (st.unresolved) resolve();
-                    if (set == 0 || t + 1 < ntiles) {  // this range's carry -> the other set
+                    if (set == 0 || t + 1 < nt) {  // this range's carry -> the other set
                         sts_f32(mail_out, st.m);
                         __syncwarp();
                         if (lane == 0) mbar_arrive(carry_out);
                     }
                 }
-                if (tr) TRACED(2 + mb, t, 6);
+                if (tr) TRACED(trole, t, 6);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
@@ -1072,7 +1119,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             if (slot >= nacc) slot -= nacc;
             if (++g == NSEG) { g = 0; gph ^= 1; }
         }
-        if (st.np) drain(pend, st.np, out, B, cfg, lane);
+        if (st.np) drain(pend, st.np, out, B, cfg, ring, lane);
     }
 
     // ---- teardown --------------------------------------------------------------------------------------------
@@ -1156,7 +1203,7 @@ struct Plan {
 
 uint32_t fixed_smem(int MB, int nset) {
     const uint32_t warps = (uint32_t)nset * 4u * MB;
-    return (uint32_t)sizeof(SegInfo) * NSEG + warps * PEND * (PEND_PITCH + 1) * 4 +
+    return (uint32_t)sizeof(SegInfo) * NSEG + DOCRING * 4 + warps * PEND * (PEND_PITCH + 1) * 4 +
            2 * 8 * 32 * 4 + 8u * (2 * MAX_STAGES + 8 + MAX_ACC + 2 * NSEG + 2 * MAX_RAW + 4 + 16) + 4 * 8 + 1024 /* alignment slack */;
 }
 
