@@ -74,10 +74,14 @@ typedef enum {
  * workspace     device scratch of at least tms_maxsim_workspace_bytes(...) bytes, 16-byte aligned; may be
  *               NULL when that size is 0 (it is 0 for Nq <= 32).  Longer queries are scored as n equal parts
  *               of Nq/n <= 32 tokens (n = Nq/32 for multiples of 32) whose partial scores (fp32 [Q*n, B])
- *               live in the workspace and are added by a second kernel; without the workspace such shapes
- *               take the general CUDA-core kernel.
- * Every document embedding is read from HBM once per group of up to 256 query rows (Q*Nq, with Nq
- * rounded up to a power of two); no similarity matrix is written to memory (Eq. 7).
+ *               live in the workspace and are added by a second kernel.  A workspace that is missing or too
+ *               small for such a shape is TMS_ERR_WORKSPACE, a mis-aligned one TMS_ERR_ALIGNMENT -- the call
+ *               never switches to a slower kernel because of its scratch.
+ * Every document embedding is read from HBM once per group of query rows that fits tensor memory next to
+ * its accumulators: 256 rows (Q*Nq, Nq rounded up to a power of two) for d*sizeof(dtype) <= 512 bytes, 128 rows
+ * beyond that (16-bit d in (256, 768], where the query block alone takes 192..384 of the 512 columns); a call with
+ * more rows runs ceil(rows / group) launches, each streaming the store once -- the ceil(Nq/BQ) factor of Thm 1
+ * (P:L228).  No similarity matrix is written to memory (Eq. 7).
  * d > 128 accumulates partial dot products over dimension chunks before the max is taken.
  */
 int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
@@ -91,6 +95,12 @@ int tms_maxsim_variant(const void* queries, int Q, int Nq, int d, const void* do
                        size_t workspace_bytes, void* stream, tms_variant variant);
 
 size_t tms_maxsim_workspace_bytes(int Q, int Nq, int d, int64_t B, tms_dtype dtype);
+
+/* Which kernel tms_maxsim (TMS_VARIANT_AUTO) runs for this shape on an sm_100 device, given an adequate workspace:
+ * TMS_VARIANT_TCGEN05 or TMS_VARIANT_SIMT (the general CUDA-core kernel, far below the HBM roofline: d*sizeof(dtype)
+ * beyond tensor-memory residency, fp32 with d % 64 != 0, total_tokens >= 2^31 - 128).  TMS_VARIANT_AUTO when nothing
+ * is scored (B == 0 or total_tokens == 0).  A pure function of its arguments: no device is touched. */
+int tms_maxsim_variant_used(int Q, int Nq, int d, int64_t B, int64_t total_tokens, tms_dtype dtype);
 
 /*
  * PQ distance table (Eq. 8):
@@ -144,7 +154,9 @@ int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_
  * and return only after the scores have landed in `scores` (they synchronise `stream`).
  *
  * dev_workspace   device memory, at least *_host_workspace_min_bytes(..., max_doc_tokens) bytes where
- *                 max_doc_tokens is the longest document; a larger workspace means fewer, larger chunks.
+ *                 max_doc_tokens is the longest document; a larger workspace means fewer, larger chunks.  The
+ *                 scratch of queries longer than 32 tokens is carved out of it (per chunk), so every shape runs the
+ *                 same kernel as through the device entry point.
  *                 TMS_ERR_WORKSPACE if a single document does not fit in half of what remains after the
  *                 query (and, for PQ, table) staging area.
  * tms_pq_maxsim_host builds the distance table on the device from host `queries` and `codebooks` first.
@@ -157,9 +169,17 @@ int tms_pq_maxsim_host(const void* queries, int Q, int Nq, int d, tms_dtype q_dt
                        int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
                        float* scores, void* dev_workspace, size_t dev_workspace_bytes, void* stream);
 
+/* tms_pq_maxsim_decode from host buffers (same shapes as tms_pq_maxsim_decode; no table is built). */
+int tms_pq_maxsim_decode_host(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks,
+                              int M, int K, const uint8_t* codes, const int64_t* offsets, int64_t B,
+                              int64_t total_tokens, float* scores, void* dev_workspace, size_t dev_workspace_bytes,
+                              void* stream);
+
 size_t tms_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype dtype, int64_t max_doc_tokens);
 size_t tms_pq_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype q_dtype, int M, int K,
                                               int64_t max_doc_tokens);
+size_t tms_pq_maxsim_decode_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype q_dtype, int M, int K,
+                                                     int64_t max_doc_tokens);
 
 /*
  * Per-query top-k over a score matrix -- the step right after scoring ("followed by torch.topk"):
@@ -168,7 +188,8 @@ size_t tms_pq_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype q_
  * scores   device, fp32 [Q, B] row-major (as written by tms_maxsim / tms_pq_maxsim); not modified; no NaN.
  * values   device, fp32 [Q, k];   indices  device, int64 [Q, k];   1 <= k <= min(B, 1024);  B <= 2^31.
  * workspace  device scratch of at least tms_topk_workspace_bytes(Q, B, k) bytes, 8-byte aligned (0 for B <= 4096).
- * Values are exact copies of the scores; the result is unique and bit-reproducible.
+ * Values are copies of the scores (a score of -0.0 ties with and is reported as +0.0); the result is unique and
+ * bit-reproducible.
  */
 int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
              size_t workspace_bytes, void* stream);

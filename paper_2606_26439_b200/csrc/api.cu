@@ -37,6 +37,17 @@ const DeviceInfo* device_info() {
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+__global__ void fill_neg_inf_kernel(float* __restrict__ x, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) x[i] = -INFINITY;
+}
+// every document is empty: all scores are -inf (Alg. 3 line 4 summed Nq times; reading A2)
+static int fill_empty(float* scores, int64_t n, cudaStream_t stream) {
+    fill_neg_inf_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(scores, n);
+    count_launch();
+    return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
+}
+
 static int check_dense(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
                        int64_t T, tms_dtype dtype, float* scores) {
     if (Q <= 0 || Nq <= 0 || d <= 0 || B < 0 || T < 0) return TMS_ERR_INVALID_ARG;
@@ -55,15 +66,31 @@ static int dense_dispatch(const void* queries, int Q, int Nq, int d, const void*
                           size_t workspace_bytes, void* stream, tms_variant variant) {
     int st = check_dense(queries, Q, Nq, d, docs, offsets, B, T, dtype, scores);
     if (st != TMS_OK) return st;
+    if (variant != TMS_VARIANT_AUTO && variant != TMS_VARIANT_SIMT && variant != TMS_VARIANT_TCGEN05)
+        return TMS_ERR_INVALID_ARG;
     if (!device_info()) return TMS_ERR_CUDA;
     if (B == 0) return TMS_OK;
-    DenseArgs a{queries, Q, Nq, d, docs, offsets, B, T, dtype, scores, static_cast<cudaStream_t>(stream),
-                aligned16(workspace) ? workspace : nullptr, workspace_bytes};
+    if (T == 0) return fill_empty(scores, (int64_t)Q * B, static_cast<cudaStream_t>(stream));  // every document empty (A2)
+    // The long-query scratch is never optional: a missing, short or mis-aligned workspace is an error, not a reason
+    // to run a slower kernel behind the caller's back.
+    const size_t need = dense_tc_workspace_bytes(Q, Nq, B);
+    DenseArgs a{queries, Q, Nq, d, docs, offsets, B, T, dtype, scores, static_cast<cudaStream_t>(stream), workspace,
+                workspace_bytes};
+    if (variant != TMS_VARIANT_SIMT && need != 0) {
+        a.workspace = reinterpret_cast<void*>(static_cast<uintptr_t>(16));  // "present" for the shape test below
+        a.workspace_bytes = need;
+        const bool tc = dense_tc_supports(a);
+        a.workspace = workspace;
+        a.workspace_bytes = workspace_bytes;
+        if (tc) {
+            if (!workspace || workspace_bytes < need) return TMS_ERR_WORKSPACE;
+            if (!aligned16(workspace)) return TMS_ERR_ALIGNMENT;
+        }
+    }
     switch (variant) {
         case TMS_VARIANT_AUTO: return dense_tc_supports(a) ? launch_dense_tc(a) : launch_dense_simt(a);
         case TMS_VARIANT_SIMT: return launch_dense_simt(a);
-        case TMS_VARIANT_TCGEN05: return dense_tc_supports(a) ? launch_dense_tc(a) : TMS_ERR_UNSUPPORTED;
-        default: return TMS_ERR_INVALID_ARG;
+        default: return dense_tc_supports(a) ? launch_dense_tc(a) : TMS_ERR_UNSUPPORTED;
     }
 }
 
@@ -113,6 +140,14 @@ int tms_maxsim_variant(const void* queries, int Q, int Nq, int d, const void* do
                        size_t workspace_bytes, void* stream, tms_variant variant) {
     return dense_dispatch(queries, Q, Nq, d, docs, offsets, B, total_tokens, dtype, scores, workspace, workspace_bytes,
                           stream, variant);
+}
+
+int tms_maxsim_variant_used(int Q, int Nq, int d, int64_t B, int64_t total_tokens, tms_dtype dtype) {
+    if (Q <= 0 || Nq <= 0 || d <= 0 || B <= 0 || total_tokens <= 0) return TMS_VARIANT_AUTO;  // nothing is scored
+    DenseArgs a{reinterpret_cast<const void*>(static_cast<uintptr_t>(16)), Q, Nq, d,
+                reinterpret_cast<const void*>(static_cast<uintptr_t>(16)), nullptr, B, total_tokens, dtype, nullptr,
+                nullptr, reinterpret_cast<void*>(static_cast<uintptr_t>(16)), dense_tc_workspace_bytes(Q, Nq, B)};
+    return dense_tc_shape_ok(a) ? TMS_VARIANT_TCGEN05 : TMS_VARIANT_SIMT;
 }
 
 size_t tms_maxsim_workspace_bytes(int Q, int Nq, int d, int64_t B, tms_dtype dtype) {
@@ -166,8 +201,14 @@ int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_
         return TMS_ERR_ALIGNMENT;
     if (!device_info()) return TMS_ERR_CUDA;
     if (B == 0) return TMS_OK;
+    if (total_tokens == 0) return fill_empty(scores, (int64_t)Q * B, static_cast<cudaStream_t>(stream));
+    const size_t need = dense_tc_workspace_bytes(Q, Nq, B);
+    if (need != 0) {
+        if (!workspace || workspace_bytes < need) return TMS_ERR_WORKSPACE;
+        if (!aligned16(workspace)) return TMS_ERR_ALIGNMENT;
+    }
     DenseArgs a{queries, Q, Nq, d, nullptr, offsets, B, total_tokens, q_dtype, scores, static_cast<cudaStream_t>(stream),
-                aligned16(workspace) ? workspace : nullptr, workspace_bytes};
+                workspace, workspace_bytes};
     a.codes = codes;
     a.codebooks = codebooks;
     return dense_tc_supports(a) ? launch_dense_tc(a) : TMS_ERR_UNSUPPORTED;

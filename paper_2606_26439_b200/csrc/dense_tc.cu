@@ -1310,6 +1310,11 @@ size_t dense_tc_workspace_bytes(int Q, int Nq, int64_t B) {
     return sizeof(float) * (size_t)Q * (size_t)query_parts(Nq) * (size_t)B;
 }
 
+bool dense_tc_shape_ok(const DenseArgs& a) {
+    Plan pl;
+    return plan(a, pl) && pl.smem_bytes <= SMEM_LIMIT;
+}
+
 bool dense_tc_supports(const DenseArgs& a) {
     const DeviceInfo* di = device_info();
     if (!di || di->cc_major != 10) return false;

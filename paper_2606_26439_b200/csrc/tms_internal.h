@@ -44,6 +44,8 @@ struct DenseArgs {
 int launch_dense_simt(const DenseArgs& a);
 // TMA + tcgen05 kernel (csrc/dense_tc.cu). supports() says whether the shape is covered.
 bool dense_tc_supports(const DenseArgs& a);
+// the shape test alone (no device query): what an sm_100 device with 227 KB of shared memory would run
+bool dense_tc_shape_ok(const DenseArgs& a);
 int launch_dense_tc(const DenseArgs& a);
 // Scratch the tcgen05 path needs for this shape (0 for Nq <= 32).
 size_t dense_tc_workspace_bytes(int Q, int Nq, int64_t B);

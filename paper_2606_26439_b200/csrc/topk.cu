@@ -16,7 +16,8 @@ constexpr int CHUNK = 4096;
 constexpr int THREADS = 1024;
 
 __device__ __forceinline__ uint64_t make_key(float score, uint32_t idx) {
-    const uint32_t b = __float_as_uint(score);
+    uint32_t b = __float_as_uint(score);
+    if (b == 0x80000000u) b = 0;  // -0.0 ties with +0.0 (equal values are ranked by index)
     const uint32_t u = (b & 0x80000000u) ? ~b : (b | 0x80000000u);  // monotone: larger float -> larger u
     return ((uint64_t)u << 32) | (uint64_t)(~idx);                   // lower index wins a tie
 }

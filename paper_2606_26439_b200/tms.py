@@ -26,6 +26,7 @@ SIGNATURES = {
     "tms_maxsim": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
     "tms_maxsim_variant": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp, _i]),
     "tms_maxsim_workspace_bytes": (_sz, [_i, _i, _i, _i64, _i]),
+    "tms_maxsim_variant_used": (_i, [_i, _i, _i, _i64, _i64, _i]),
     "tms_pq_build_lut": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp]),
     "tms_pq_maxsim": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
@@ -33,6 +34,8 @@ SIGNATURES = {
     "tms_pq_maxsim_decode": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_maxsim_host": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
+    "tms_pq_maxsim_decode_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
+    "tms_pq_maxsim_decode_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i, _i, _i64]),
     "tms_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i64]),
     "tms_pq_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i, _i, _i64]),
     "tms_topk": (_i, [_vp, _i, _i64, _i, _vp, _vp, _vp, _sz, _vp]),
@@ -87,6 +90,12 @@ def tms_version() -> int:
 
 def tms_maxsim_workspace_bytes(Q, Nq, d, B, dtype) -> int:
     return int(load().tms_maxsim_workspace_bytes(Q, Nq, d, B, _DTYPES[dtype]))
+
+
+def tms_maxsim_variant_used(Q, Nq, d, B, total_tokens, dtype) -> str:
+    """Name of the kernel tms_maxsim picks for this shape ("tcgen05" / "simt"; "auto" when nothing is scored)."""
+    v = int(load().tms_maxsim_variant_used(Q, Nq, d, B, total_tokens, _DTYPES[dtype]))
+    return {val: name for name, val in VARIANTS.items()}[v]
 
 
 def tms_topk_workspace_bytes(Q, B, k) -> int:
@@ -247,4 +256,23 @@ def tms_pq_maxsim_host(queries: torch.Tensor, codebooks: torch.Tensor, codes: to
                                    _dev(dev_workspace, "dev_workspace"),
                                    dev_workspace.numel() * dev_workspace.element_size(), _stream(stream))
     _check(st, "tms_pq_maxsim_host")
+    return scores
+
+
+def tms_pq_maxsim_decode_host_workspace_min_bytes(Q, Nq, d, q_dtype, M, K, max_doc_tokens) -> int:
+    return int(load().tms_pq_maxsim_decode_host_workspace_min_bytes(Q, Nq, d, _DTYPES[q_dtype], M, K, max_doc_tokens))
+
+
+def tms_pq_maxsim_decode_host(queries: torch.Tensor, codebooks: torch.Tensor, codes: torch.Tensor,
+                              offsets: torch.Tensor, scores: torch.Tensor, dev_workspace: torch.Tensor,
+                              stream=None) -> torch.Tensor:
+    Q, Nq, d = queries.shape
+    M, K, _ = codebooks.shape
+    T, B = codes.shape[0], offsets.numel() - 1
+    st = load().tms_pq_maxsim_decode_host(_host(queries, "queries"), Q, Nq, d, _DTYPES[queries.dtype],
+                                          _host(codebooks, "codebooks"), M, K, _host(codes, "codes"),
+                                          _host(offsets, "offsets"), B, T, _host(scores, "scores"),
+                                          _dev(dev_workspace, "dev_workspace"),
+                                          dev_workspace.numel() * dev_workspace.element_size(), _stream(stream))
+    _check(st, "tms_pq_maxsim_decode_host")
     return scores
