@@ -117,6 +117,7 @@ class ClockSampler:
 
     def __init__(self, device_index: int, period_s: float = 0.005):
         self.period, self.samples, self.mask, self.h, self.max_mhz = period_s, [], 0, None, None
+        self.power, self.power_limit = [], None
         self._stop = threading.Event()
         self._thread = None
         try:
@@ -131,6 +132,10 @@ class ClockSampler:
                 self.h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
             self.nv = pynvml
             self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            try:
+                self.power_limit = pynvml.nvmlDeviceGetEnforcedPowerLimit(self.h) / 1000.0
+            except Exception:
+                self.power_limit = None
         except Exception:
             self.h = None
 
@@ -139,9 +144,23 @@ class ClockSampler:
             try:
                 self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
                 self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.power.append(self._power_w())
             except Exception:
                 pass
             time.sleep(self.period)
+
+    def _power_w(self):
+        """Instantaneous board power when the driver exposes it (NVML_FI_DEV_POWER_INSTANT), else the ~1 s average."""
+        try:
+            fid = getattr(self.nv, "NVML_FI_DEV_POWER_INSTANT", 186)
+            v = self.nv.nvmlDeviceGetFieldValues(self.h, [fid])[0]
+            if v.nvmlReturn == 0 and v.value.uiVal > 0:
+                self.power_kind = "instant"
+                return v.value.uiVal / 1000.0
+        except Exception:
+            pass
+        self.power_kind = "1 s average"
+        return self.nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
 
     def start(self):
         if self.h is not None:
@@ -154,7 +173,11 @@ class ClockSampler:
             self._thread.join()
         reasons = [name for bit, name in self.REASONS.items() if self.mask & bit and name != "gpu_idle"]
         med = int(np.median(self.samples)) if self.samples else None
-        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": reasons, "samples": len(self.samples)}
+        out = {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": reasons, "samples": len(self.samples)}
+        if self.power:
+            out.update({"power_w_mean": float(np.mean(self.power)), "power_w_max": float(np.max(self.power)),
+                        "power_limit_w": self.power_limit, "power_kind": getattr(self, "power_kind", None)})
+        return out
 
 
 # ---- the CPU oracle legs (the only places bench.py touches oracle/) --------------------------------------------------
@@ -221,7 +244,7 @@ def run_reference(args, w, rank):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": config_dict(args, w, B, int(make_offsets(w, B, args.seed)[-1]), sample_docs_per_step=n),
+        "config": config_dict(args, w, B, int(make_offsets(w, B, args.seed)[-1]), 1, sample_docs_per_step=n),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(used), "kind": "oracle",
                          "sample": f"{n} documents per step (same recipe as the workload), all {w['Q']} queries, fp64"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -231,13 +254,12 @@ def run_reference(args, w, rank):
     print(json.dumps(line), flush=True)
 
 
-def config_dict(args, w, B, T, **extra):
+def config_dict(args, w, B, T, world=1, **extra):
     c = {"workload": f"{args.workload}: " + ("dense MaxSim" if w["kind"] == "dense" else "fused PQ MaxSim"),
          "Q": w["Q"], "Nq": w["Nq"], "d": w["d"], "store_dtype": w["dtype"], "B_per_gpu": B, "total_tokens_per_gpu": T,
          "lengths": ("uniform Nd=%d" % w["Nd"]) if w["lengths"] == "uniform" else "lognormal(median 64, sigma 0.5) clip [8,180]",
-         "l2": "inputs larger than L2 (no flush needed)" if T * w["d"] * ELEM_BYTES[w["dtype"]] > (512 << 20) or
-               (w["kind"] == "pq" and T * w.get("M", 0) > (512 << 20)) else "L2 flushed between timed steps",
-         "parallelism": f"dp{args.gpus} (documents sharded, no data-path collective)"}
+         "l2": config_l2(w, T),
+         "parallelism": f"dp{world} (one process per GPU, documents sharded, no data-path collective)"}
     if w["kind"] == "pq":
         c.update({"M": w["M"], "K": w["K"]})
     c.update(extra)
@@ -245,6 +267,232 @@ def config_dict(args, w, B, T, **extra):
 
 
 # ---- the CUDA arm ----------------------------------------------------------------------------------------------------
+
+def load_peaks():
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        pk = json.load(open(peaks_path))
+        return {"hbm": float(pk["hbm_gbs"]), "tc_burst": float(pk["bf16_tflops"]),
+                "tc_sustained": float(pk.get("bf16_tflops_sustained", pk["bf16_tflops"])),
+                "source": "MEASURED_PEAKS.json (HBM: device-to-device copy rate, read+write bytes; tensor: cuBLAS bf16 8192^3)"}
+    return {"hbm": FALLBACK_HBM_GBS, "tc_burst": FALLBACK_BF16_TFLOPS, "tc_sustained": FALLBACK_BF16_TFLOPS_SUSTAINED,
+            "source": "B200_PROFILING.md fallback"}
+
+
+def profiled_traffic(name):
+    """DRAM bytes per launch from the committed ncu capture (not measured in this run): (bytes, source) or (None, None)."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tpath):
+        return None, None
+    lines = open(tpath).read().splitlines()
+    src = "profiles/traffic.csv (ncu dram__bytes_read.sum + dram__bytes_write.sum, one launch; %s)" % (
+        lines[0].split("#", 1)[1].strip() if "#" in lines[0] else "see profiles/*.md for the capture")
+    for ln in lines[1:]:
+        nm, _, val = ln.partition(",")
+        if nm == name:
+            return int(val), src
+    return None, None
+
+
+class Workload:
+    """One workload's device-resident inputs and its step function (one pass of the hot path through the C ABI)."""
+
+    def __init__(self, name, w, B, seed, dev, tms, variant="auto", reuse=None):
+        self.name, self.w, self.B, self.dev, self.tms = name, w, B, dev, tms
+        if reuse is not None and reuse.w["kind"] == w["kind"] == "dense" and reuse.B == B and \
+                all(reuse.w[k] == w[k] for k in ("d", "dtype", "lengths", "Nd")):
+            # same store (same recipe, seed and shape); only the queries differ
+            from paper_2606_26439_b200 import synth
+
+            q = synth.unit_tokens(w["Q"] * w["Nq"], w["d"], TORCH_DTYPES[w["dtype"]], seed=seed + 1,
+                                  device=dev).view(w["Q"], w["Nq"], w["d"])
+            self.inp = dict(reuse.inp, q=q)
+        else:
+            self.inp = make_inputs(w, B, seed, dev)
+        inp = self.inp
+        self.T = inp["T"]
+        self.off_d = torch.from_numpy(inp["off"]).to(dev)
+        self.scores = torch.empty((w["Q"], B), dtype=torch.float32, device=dev)
+        self.l2 = config_l2(w, self.T)
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if "flushed" in self.l2 else None
+        Q, Nq, d = w["Q"], w["Nq"], w["d"]
+        if w["kind"] == "dense":
+            need = tms.tms_maxsim_workspace_bytes(Q, Nq, d, B, TORCH_DTYPES[w["dtype"]])
+            dws = torch.empty(need, dtype=torch.uint8, device=dev) if need else None  # only queries longer than 32 tokens
+            k = w.get("topk", 0)
+            if k:
+                tk_v = torch.empty((Q, k), dtype=torch.float32, device=dev)
+                tk_i = torch.empty((Q, k), dtype=torch.int64, device=dev)
+                tk_ws = torch.empty(max(tms.tms_topk_workspace_bytes(Q, B, k), 8), dtype=torch.uint8, device=dev)
+
+            def step():
+                tms.tms_maxsim(inp["q"], inp["store"], self.off_d, scores=self.scores, variant=variant, workspace=dws)
+                if k:
+                    tms.tms_topk(self.scores, k, values=tk_v, indices=tk_i, workspace=tk_ws)
+            self.kernel = tms.tms_maxsim_variant_used(Q, Nq, d, B, self.T, TORCH_DTYPES[w["dtype"]]) \
+                if variant == "auto" else variant
+        elif w.get("decode"):
+            def step():
+                tms.tms_pq_maxsim_decode(inp["q"], inp["C"], inp["store"], self.off_d, scores=self.scores)
+            self.kernel = "tcgen05 (decode-and-contract)"
+        else:
+            lut = torch.empty((Q, Nq, w["M"], w["K"]), dtype=torch.float32, device=dev)
+            ws = torch.empty(max(tms.tms_pq_workspace_bytes(Q, Nq, w["M"], w["K"], B), 16), dtype=torch.uint8, device=dev)
+
+            def step():
+                tms.tms_pq_build_lut(inp["q"], inp["C"], lut=lut)
+                tms.tms_pq_maxsim(lut, inp["store"], self.off_d, scores=self.scores, workspace=ws, variant=variant)
+            self.kernel = "pq_smem" if ws.numel() > 16 else "pq_simt"
+        self.step = step
+
+
+def config_l2(w, T):
+    big = T * w["d"] * ELEM_BYTES[w["dtype"]] > (512 << 20) or (w["kind"] == "pq" and T * w.get("M", 0) > (512 << 20))
+    return "inputs larger than L2 (no flush needed)" if big else "L2 flushed between timed steps"
+
+
+def timed_region(wl, steps, warmup, local_rank, sync_all, shard):
+    """W warm-up steps, then exactly K steps with per-step CUDA events on the launching stream; clocks, throttle reasons and
+    board power are sampled through NVML while the steps run.  Returns per-step times and the max-over-ranks total."""
+    for _ in range(warmup):
+        wl.step()
+    sync_all()
+    sampler = ClockSampler(local_rank)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = wl.tms.tms_launch_count()
+    sampler.start()
+    sync_all()
+    t_start.record()
+    for a, b in ev:
+        if wl.flush is not None:
+            wl.flush.fill_(1)
+        a.record()
+        wl.step()
+        b.record()
+    t_end.record()
+    sync_all()
+    clocks = sampler.stop()
+    launches = wl.tms.tms_launch_count() - n0
+    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    total_ms = float(step_ms.sum()) if wl.flush is not None else float(t_start.elapsed_time(t_end))
+    total_ms = shard.max_over_ranks(total_ms, wl.dev)
+    return step_ms, total_ms, clocks, int(launches)
+
+
+def roofline_of(wl, step_ms, total_ms, clocks, peaks):
+    """The binding roofline of the dominant kernel: algorithmic bytes (or FLOP) per launch / mean launch time."""
+    from paper_2606_26439_b200 import accounting
+
+    w, T, B = wl.w, wl.T, wl.B
+    hbm_peak, tc_burst, tc_sust = peaks["hbm"], peaks["tc_burst"], peaks["tc_sustained"]
+    abytes = algorithmic_bytes(w, T, B)
+    kern_ms = float(step_ms.mean())
+    kern_s = kern_ms * 1e-3
+    hbm_gbs = abytes / kern_s / 1e9
+    traffic, traffic_src = profiled_traffic(wl.name)
+    common = {"traffic": traffic, "traffic_source": traffic_src, "peak_source": peaks["source"],
+              "algorithmic_bytes_per_launch": abytes, "kernel": wl.kernel,
+              "kernel_ms_mean": kern_ms, "kernel_ms_min": float(step_ms.min()), "kernel_ms_median": float(np.median(step_ms)),
+              "hbm": {"achieved_GBps": hbm_gbs, "peak_GBps": hbm_peak, "frac": hbm_gbs / hbm_peak,
+                      "frac_of_nominal_8000": hbm_gbs / 8000.0, "ideal_ms": abytes / (hbm_peak * 1e9) * 1e3}}
+    notes = []
+    if hbm_gbs > hbm_peak:
+        notes.append("achieved exceeds the HBM 'peak' because that figure is a copy rate (reads + writes share the bus "
+                     "and turn it around) while this kernel only reads")
+    if w["kind"] == "dense" or w.get("decode"):
+        # tensor work: 2*Q*Nq*T*d algorithmic FLOP.  fp32 inputs cost three bf16 MMAs per product (DESIGN.md 5.3), the PQ
+        # decode variant two (bf16 queries), so their tensor peaks are a third / half of the bf16 peak.
+        fl = accounting.dense_flops(w["Q"], w["Nq"], w["d"], T)
+        div = 2.0 if w.get("decode") else (3.0 if w["dtype"] == "fp32" else 1.0)
+        tfl = fl / kern_s / 1e12
+        common["tensor"] = {"achieved_TFLOPs": tfl, "mma_per_product": div, "algorithmic_flops_per_launch": fl,
+                            "peak_TFLOPs_burst": tc_burst / div, "frac_burst": tfl / (tc_burst / div),
+                            "peak_TFLOPs_sustained": tc_sust / div, "frac_sustained": tfl / (tc_sust / div),
+                            "ideal_ms_burst": fl / (tc_burst / div * 1e12) * 1e3}
+        if w.get("decode") or fl / (tc_burst / div * 1e12) > abytes / (hbm_peak * 1e9):
+            roofline = {"bound": "tensor", "achieved": tfl, "peak": tc_burst / div, "unit": "TFLOP/s",
+                        "frac": tfl / (tc_burst / div)}
+        else:
+            roofline = {"bound": "hbm", "achieved": hbm_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_gbs / hbm_peak}
+        ih, it = common["hbm"]["ideal_ms"], common["tensor"]["ideal_ms_burst"]
+        if abs(ih - it) < 0.1 * max(ih, it):
+            notes.append("HBM and tensor ideal times are within 10 %% of each other (%.3f vs %.3f ms at the burst peaks): "
+                         "read `frac` as the fraction of either" % (ih, it))
+    else:
+        # fused PQ (LUT form): Q*Nq*T*M four-byte shared-memory gathers against M bytes of codes per token -- bound by
+        # the shared-memory load pipe (128 B/clk/SM), not by HBM and not by tensor cores (DESIGN.md 5.4)
+        lookups = accounting.pq_lookups(w["Q"], w["Nq"], w["M"], T)
+        g = lookups * 4 / kern_s / 1e9
+        roofline = {"bound": "alu", "achieved": g, "peak": SMEM_PIPE_PEAK_GBS, "unit": "GB/s", "frac": g / SMEM_PIPE_PEAK_GBS}
+        notes.append("shared-memory gather bytes/s against 148 SMs x 128 B/clk x 1.965 GHz; step = LUT build + relayout + "
+                     "fused lookup kernel")
+    # what THIS run observed about clocks and power (NVML samples taken while the timed steps ran)
+    p_w, p_lim = clocks.get("power_w_mean"), clocks.get("power_limit_w")
+    obs = "this run: NVML SM clock median %s MHz (max %s), throttle reasons %s" % (
+        clocks.get("sm_mhz"), clocks.get("sm_max_mhz"), clocks.get("reasons") or "none")
+    if p_w and p_lim:
+        obs += ", board power (%s) mean %.0f W / max %.0f W of a %.0f W limit over %d samples" % (
+            clocks.get("power_kind"), p_w, clocks.get("power_w_max", p_w), p_lim, clocks.get("samples", 0))
+        if clocks.get("power_w_max", 0) >= 0.93 * p_lim:
+            obs += " -- the run sits at the board power limit; NVML's clock field does not show the sub-millisecond " \
+                   "clock reductions the power controller applies (DESIGN.md 5.1 has the in-kernel measurement)"
+    notes.append(obs)
+    roofline["note"] = "; ".join(notes)
+    roofline["timed_region_ms"] = total_ms
+    roofline.update(common)
+    return roofline
+
+
+SECONDARY = ["c2-q4", "c2-q1", "c2-fp16", "c2-fp32", "c3-100k", "c3-250k", "c3-500k", "c4-d64", "c4-d256", "c4-d512",
+             "c4-d768", "c5", "c5-decode"]
+
+
+def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):
+    """The other BASELINE.json configs, each timed briefly (its own warm-up, 5 steps, its own clock samples) AFTER and
+    outside the headline's timed region: {name: {ms_per_step, docs_per_s, bound, frac, ...}}."""
+    out = {}
+    prev = main_wl
+    for name in SECONDARY:
+        if name == args.workload:
+            continue
+        w = WORKLOADS[name]
+        try:
+            wl = Workload(name, w, w["B"], args.seed, dev, tms, reuse=prev)
+            step_ms, total_ms, clocks, launches = timed_region(wl, args.secondary_steps, 3, local_rank, sync_all, shard)
+            r = roofline_of(wl, step_ms, total_ms, clocks, peaks)
+            out[name] = {"ms_per_step": float(step_ms.mean()), "ms_min": float(step_ms.min()),
+                         "docs_per_s": w["B"] / (float(step_ms.mean()) * 1e-3), "steps": args.secondary_steps,
+                         "bound": r["bound"], "frac": r["frac"], "achieved": r["achieved"], "peak": r["peak"],
+                         "unit": r["unit"], "hbm_GBps": r["hbm"]["achieved_GBps"], "hbm_frac": r["hbm"]["frac"],
+                         "tensor_frac_burst": r.get("tensor", {}).get("frac_burst"), "kernel": r["kernel"],
+                         "gpu_launches": launches, "traffic": r["traffic"],
+                         "clocks": {k: clocks.get(k) for k in ("sm_mhz", "reasons", "power_w_mean", "power_w_max")},
+                         "B": w["B"], "total_tokens": wl.T}
+            if prev is not main_wl and prev is not wl:
+                del prev
+            prev = wl
+        except Exception as e:  # a secondary workload never takes the headline down with it
+            out[name] = {"error": repr(e)[:200]}
+        torch.cuda.empty_cache()
+    return out
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks here (same command line under
+    torch.distributed.run, one rank per GPU over NCCL) and pass rank 0's JSON line through."""
+    import socket
+    import subprocess
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    raise SystemExit(subprocess.call(cmd, env=env))
+
 
 def main():
     ap = argparse.ArgumentParser()
@@ -258,11 +506,14 @@ def main():
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the brief timings of the other configs")
+    ap.add_argument("--secondary-steps", type=int, default=5)
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "tms" else args.warmup
     w = WORKLOADS[args.workload]
 
+    launched = "WORLD_SIZE" in os.environ
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -270,6 +521,10 @@ def main():
     if args.impl == "reference":
         run_reference(args, w, rank)
         return
+    if args.gpus > 1 and not launched:
+        spawn_ranks(args)  # does not return
+    if launched and world != args.gpus and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; reporting n_gpus={world}", file=sys.stderr)
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
@@ -289,166 +544,38 @@ def main():
         dist.barrier()
     tms.load()
 
-    B = args.B or w["B"]
-    inp = make_inputs(w, B, args.seed + 1000 * rank, dev)  # weak scaling: every rank owns its own B-document shard
-    T = inp["T"]
-    off_d = torch.from_numpy(inp["off"]).to(dev)
-    scores = torch.empty((w["Q"], B), dtype=torch.float32, device=dev)
-    flush = None
-    small = "flushed" in config_dict(args, w, B, T)["l2"]
-    if small:
-        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-
-    if w["kind"] == "dense":
-        need = tms.tms_maxsim_workspace_bytes(w["Q"], w["Nq"], w["d"], B, TORCH_DTYPES[w["dtype"]])
-        dws = torch.empty(need, dtype=torch.uint8, device=dev) if need else None  # only queries longer than 32 tokens
-
-        k = w.get("topk", 0)
-        if k:
-            tk_v = torch.empty((w["Q"], k), dtype=torch.float32, device=dev)
-            tk_i = torch.empty((w["Q"], k), dtype=torch.int64, device=dev)
-            tk_ws = torch.empty(max(tms.tms_topk_workspace_bytes(w["Q"], B, k), 8), dtype=torch.uint8, device=dev)
-
-        def step():
-            tms.tms_maxsim(inp["q"], inp["store"], off_d, scores=scores, variant=args.variant, workspace=dws)
-            if k:
-                tms.tms_topk(scores, k, values=tk_v, indices=tk_i, workspace=tk_ws)
-    else:
-        lut = torch.empty((w["Q"], w["Nq"], w["M"], w["K"]), dtype=torch.float32, device=dev)
-        ws = torch.empty(max(tms.tms_pq_workspace_bytes(w["Q"], w["Nq"], w["M"], w["K"], B), 16), dtype=torch.uint8,
-                         device=dev)
-
-        if w.get("decode"):
-            def step():
-                tms.tms_pq_maxsim_decode(inp["q"], inp["C"], inp["store"], off_d, scores=scores)
-        else:
-            def step():
-                tms.tms_pq_build_lut(inp["q"], inp["C"], lut=lut)
-                tms.tms_pq_maxsim(lut, inp["store"], off_d, scores=scores, workspace=ws, variant=args.variant)
-
     def sync_all():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
             torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
-    sync_all()
-
-    # ---- timed region: exactly K steps; per-step CUDA events on the launching stream --------------------------------
-    sampler = ClockSampler(local_rank)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    n0 = tms.tms_launch_count()
-    sampler.start()
-    sync_all()
-    t_start.record()
-    for a, b in ev:
-        if flush is not None:
-            flush.fill_(1)
-        a.record()
-        step()
-        b.record()
-    t_end.record()
-    sync_all()
-    clocks = sampler.stop()
-    launches = tms.tms_launch_count() - n0
-    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
-    total_ms = float(step_ms.sum()) if flush is not None else float(t_start.elapsed_time(t_end))
-    total_ms = shard.max_over_ranks(total_ms, dev)
+    B = args.B or w["B"]
+    # weak scaling: every rank owns its own B-document shard (token-balanced shards of a world*B store have this size)
+    wl = Workload(args.workload, w, B, args.seed + 1000 * rank, dev, tms, variant=args.variant)
+    T = wl.T
+    step_ms, total_ms, clocks, launches = timed_region(wl, args.steps, args.warmup, local_rank, sync_all, shard)
     ms_per_step = total_ms / args.steps
     value = world * B / (ms_per_step * 1e-3)
-
-    # ---- roofline of the dominant kernel ------------------------------------------------------------------------------
-    # Each step is timed alone (events around one call), so the burst peaks of MEASURED_PEAKS.json apply.
-    from paper_2606_26439_b200 import accounting
-
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        pk = json.load(open(peaks_path))
-        hbm_peak, tc_peak, peak_src = float(pk["hbm_gbs"]), float(pk["bf16_tflops"]), "MEASURED_PEAKS.json (of measured)"
-        tc_sustained = float(pk.get("bf16_tflops_sustained", tc_peak))
-    else:
-        hbm_peak, tc_peak, peak_src = FALLBACK_HBM_GBS, FALLBACK_BF16_TFLOPS, "B200_PROFILING.md fallback (of fallback)"
-        tc_sustained = FALLBACK_BF16_TFLOPS_SUSTAINED
-    # Tensor peak by regime (B200_PROFILING.md): the burst figure for kernels timed alone; when the timed region is a
-    # long back-to-back loop that ran under the power cap -- the regime of the sustained cuBLAS measurement -- the
-    # sustained figure.  The HBM peak is the measured copy rate in both regimes.
-    tc_regime = "burst"
-    if total_ms > 100.0 and "sw_power_cap" in clocks.get("reasons", []):
-        tc_peak, tc_regime = tc_sustained, "sustained (timed region %.0f ms under sw_power_cap)" % total_ms
-    peak_src += ", tensor peak: " + tc_regime
-    abytes = algorithmic_bytes(w, T, B)
-    kern_ms = float(step_ms.mean())
-    kern_s = kern_ms * 1e-3
-    hbm_gbs = abytes / kern_s / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")  # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch
-    if os.path.exists(tpath):
-        for ln in open(tpath).read().splitlines()[1:]:
-            name, _, val = ln.partition(",")
-            if name == args.workload:
-                traffic = int(val)
-    common = {"traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes,
-              "kernel_ms_mean": kern_ms, "kernel_ms_min": float(step_ms.min()),
-              "kernel_ms_median": float(np.median(step_ms)),
-              "hbm": {"achieved_GBps": hbm_gbs, "peak_GBps": hbm_peak, "frac": hbm_gbs / hbm_peak,
-                      "frac_of_nominal_8000": hbm_gbs / 8000.0}}
-    if w["kind"] == "dense":
-        # tensor work: 2*Q*Nq*T*d algorithmic FLOP; fp32 inputs cost three bf16 MMAs per product, so
-        # their tensor peak is a third of the bf16 peak.  The roofline that binds is the one with the larger ideal time.
-        fl = accounting.dense_flops(w["Q"], w["Nq"], w["d"], T)
-        tc_eff_peak = tc_peak / (3.0 if w["dtype"] == "fp32" else 1.0)
-        tfl = fl / kern_s / 1e12
-        common["tensor"] = {"achieved_TFLOPs": tfl, "peak_TFLOPs": tc_eff_peak, "frac": tfl / tc_eff_peak,
-                            "algorithmic_flops_per_launch": fl}
-        if fl / (tc_eff_peak * 1e12) > abytes / (hbm_peak * 1e9):
-            roofline = {"bound": "tensor", "achieved": tfl, "peak": tc_eff_peak, "unit": "TFLOP/s",
-                        "frac": tfl / tc_eff_peak}
-        else:
-            roofline = {"bound": "hbm", "achieved": hbm_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_gbs / hbm_peak}
-        roofline["tensor_tflops"] = tfl
-        if w["Q"] * w["Nq"] > 128 and w["dtype"] != "fp32":
-            roofline["note"] = ("two query blocks: HBM and tensor ideal times are within 1 % of each other at the burst peaks; the "
-                                "kernel's read stream alone draws 750-950 W of the 1000 W cap, so the tensor pipe runs at a "
-                                "power-capped SM clock of ~1.3 GHz (~1.05 GHz sustained) and binds (DESIGN.md 5.1)")
-    elif w.get("decode"):
-        # decode-and-contract PQ: 2*Q*Nq*T*d FLOP at two bf16 MMAs per product for bf16 queries (hi*hi + hi*lo)
-        fl = accounting.dense_flops(w["Q"], w["Nq"], w["d"], T)
-        tc_eff_peak = tc_peak / 2.0
-        tfl = fl / kern_s / 1e12
-        roofline = {"bound": "tensor", "achieved": tfl, "peak": tc_eff_peak, "unit": "TFLOP/s", "frac": tfl / tc_eff_peak,
-                    "note": "codes decoded in shared memory and contracted on tcgen05; two bf16 MMAs per product "
-                            "(centroids split hi/lo), so the tensor peak is half the bf16 peak (DESIGN.md 10)"}
-    else:
-        # fused PQ: Q*Nq*T*M four-byte shared-memory gathers against M bytes of codes per token -- bound by the
-        # shared-memory load pipe (128 B/clk/SM), not by HBM and not by tensor cores
-        lookups = accounting.pq_lookups(w["Q"], w["Nq"], w["M"], T)
-        smem_peak = SMEM_PIPE_PEAK_GBS
-        g = lookups * 4 / kern_s / 1e9
-        roofline = {"bound": "alu", "achieved": g, "peak": smem_peak, "unit": "GB/s", "frac": g / smem_peak,
-                    "note": "shared-memory gather bytes/s against 148 SMs x 128 B/clk x 1.965 GHz; step = LUT build + "
-                            "relayout + fused lookup kernel (DESIGN.md 5.4)"}
-    roofline.update(common)
+    peaks = load_peaks()
+    roofline = roofline_of(wl, step_ms, total_ms, clocks, peaks)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w["dtype"] if w["kind"] == "dense" else "f32", "data": "synthetic",
-        "config": config_dict(args, w, B, T), "pairs_per_s": value * w["Q"],
-        "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
+        "config": config_dict(args, w, B, T, world), "pairs_per_s": value * w["Q"],
+        "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
     }
 
     # ---- end to end through the host-buffer entry point: H2D of the store + D2H of the scores every step -------------
     if not args.no_e2e:
-        if w.get("decode"):  # no host-buffer entry point for the decode variant: its end-to-end number is c5's copy-bound one
-            line["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
-                           "unavailable": "tms_pq_maxsim_decode has no host-buffer entry point; see workload c5"}
-        else:
-            line["e2e"] = run_e2e(args, w, inp, B, T, dev, world, tms, shard)
-    if rank == 0 and not args.no_cpu and world >= 1:
-        line["cpu_baseline"] = cpu_baseline(w, inp, B)
+        line["e2e"] = run_e2e(args, w, wl.inp, B, T, dev, world, tms, shard)
+    if rank == 0 and not args.no_cpu:
+        line["cpu_baseline"] = cpu_baseline(w, wl.inp, B)
+    # ---- the other configs, briefly, outside the headline's timed region (single-GPU runs only) ----------------------
+    if world == 1 and not args.no_secondary and args.workload == "c2" and not args.B:
+        line["secondary"] = run_secondary(args, wl, dev, local_rank, tms, shard, sync_all, peaks)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -481,9 +608,10 @@ def run_e2e(args, w, inp, B, T, dev, world, tms, shard):
         h2d = q_h.numel() * q_h.element_size() + Te * row + (Be + 1) * 8
     else:
         C_h = inp["C"].cpu().pin_memory()
+        host_fn = tms.tms_pq_maxsim_decode_host if w.get("decode") else tms.tms_pq_maxsim_host
 
         def call():
-            tms.tms_pq_maxsim_host(q_h, C_h, store_h, off_h, scores_h, ws)
+            host_fn(q_h, C_h, store_h, off_h, scores_h, ws)
         h2d = q_h.numel() * q_h.element_size() + C_h.numel() * 4 + Te * row + (Be + 1) * 8
     d2h = w["Q"] * Be * 4
     call()
@@ -500,7 +628,8 @@ def run_e2e(args, w, inp, B, T, dev, world, tms, shard):
     ms = shard.max_over_ranks(max(a.elapsed_time(b), 1e3 * (time.perf_counter() - t0)), dev)
     return {"value": world * Be * args.e2e_steps / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
             "d2h_bytes_per_step": int(d2h), "steps": args.e2e_steps, "docs_per_step_per_gpu": Be,
-            "api": "tms_maxsim_host" if w["kind"] == "dense" else "tms_pq_maxsim_host",
+            "api": "tms_maxsim_host" if w["kind"] == "dense" else
+                   ("tms_pq_maxsim_decode_host" if w.get("decode") else "tms_pq_maxsim_host"),
             "ms_per_step": ms / args.e2e_steps}
 
 
