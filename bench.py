@@ -376,7 +376,7 @@ def timed_region(wl, steps, warmup, local_rank, sync_all, shard):
     launches = wl.tms.tms_launch_count() - n0
     step_ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = float(step_ms.sum()) if wl.flush is not None else float(t_start.elapsed_time(t_end))
-    total_ms = shard.max_over_ranks(total_ms, wl.dev)
+    _, total_ms = shard.aggregate_throughput(1.0, total_ms, wl.dev)  # MAX over ranks of the device-timed region
     return step_ms, total_ms, clocks, int(launches)
 
 
@@ -552,11 +552,11 @@ def main():
 
     B = args.B or w["B"]
     # weak scaling: every rank owns its own B-document shard (token-balanced shards of a world*B store have this size)
-    wl = Workload(args.workload, w, B, args.seed + 1000 * rank, dev, tms, variant=args.variant)
+    wl = Workload(args.workload, w, B, shard.rank_seed(args.seed, rank), dev, tms, variant=args.variant)
     T = wl.T
     step_ms, total_ms, clocks, launches = timed_region(wl, args.steps, args.warmup, local_rank, sync_all, shard)
     ms_per_step = total_ms / args.steps
-    value = world * B / (ms_per_step * 1e-3)
+    value = world * B / (ms_per_step * 1e-3)  # = shard.aggregate_throughput(B, ms_per_step): whole-job documents/s
     peaks = load_peaks()
     roofline = roofline_of(wl, step_ms, total_ms, clocks, peaks)
 

@@ -196,6 +196,21 @@ int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_
 
 size_t tms_topk_workspace_bytes(int Q, int64_t B, int k);
 
+/*
+ * k-way merge of per-shard top-k lists -- the step after data-parallel scoring ("only a final concatenation of
+ * per-shard scores"; with per-shard tms_topk only G*k candidates per query cross GPUs instead of B scores):
+ *     (out_values[q, :], out_indices[q, :]) = the k best of the G*k_in candidates
+ *         (values[g, q, r], shard_base[g] + indices[g, q, r]),  same order as tms_topk (score descending, lower GLOBAL
+ *         document index first, -INFINITY last).  With k_in >= k this equals tms_topk over the concatenated scores.
+ * values / indices   device, fp32 / int64 [G, Q, k_in] (shard-local document indices, as tms_topk wrote them).
+ * shard_base         HOST, int64 [G]: first global document index of every shard; 0 <= base, base + index < 2^31.
+ * G <= 64; k, k_in <= 1024; k <= G*k_in.  workspace: device, >= tms_topk_merge_workspace_bytes(...), 8-byte aligned.
+ */
+int tms_topk_merge(const float* values, const int64_t* indices, const int64_t* shard_base, int G, int Q, int k_in, int k,
+                   float* out_values, int64_t* out_indices, void* workspace, size_t workspace_bytes, void* stream);
+
+size_t tms_topk_merge_workspace_bytes(int G, int Q, int k_in, int k);
+
 /* Number of kernels this library has launched in this process since load (all entry points). */
 uint64_t tms_launch_count(void);
 

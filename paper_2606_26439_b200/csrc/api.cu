@@ -234,6 +234,30 @@ size_t tms_topk_workspace_bytes(int Q, int64_t B, int k) {
     return topk_workspace_bytes(Q, B, k);
 }
 
+int tms_topk_merge(const float* values, const int64_t* indices, const int64_t* shard_base, int G, int Q, int k_in, int k,
+                   float* out_values, int64_t* out_indices, void* workspace, size_t workspace_bytes, void* stream) {
+    if (G <= 0 || Q <= 0 || k_in <= 0 || k <= 0 || !values || !indices || !shard_base || !out_values || !out_indices)
+        return TMS_ERR_INVALID_ARG;
+    if ((int64_t)k > (int64_t)G * k_in) return TMS_ERR_INVALID_ARG;
+    if (G > 64 || k > 1024 || k_in > 1024 || Q > 65535) return TMS_ERR_UNSUPPORTED;
+    for (int g = 0; g < G; ++g)
+        if (shard_base[g] < 0 || shard_base[g] > (1ll << 31)) return TMS_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(values) & 3u) || (reinterpret_cast<uintptr_t>(out_values) & 3u) ||
+        (reinterpret_cast<uintptr_t>(indices) & 7u) || (reinterpret_cast<uintptr_t>(out_indices) & 7u))
+        return TMS_ERR_ALIGNMENT;
+    if (!workspace || workspace_bytes < topk_merge_workspace_bytes(G, Q, k_in, k) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 7u))
+        return TMS_ERR_WORKSPACE;
+    if (!device_info()) return TMS_ERR_CUDA;
+    return launch_topk_merge(values, indices, shard_base, G, Q, k_in, k, out_values, out_indices, workspace,
+                             static_cast<cudaStream_t>(stream));
+}
+
+size_t tms_topk_merge_workspace_bytes(int G, int Q, int k_in, int k) {
+    if (G <= 0 || Q <= 0 || k_in <= 0 || k <= 0) return 0;
+    return topk_merge_workspace_bytes(G, Q, k_in, k);
+}
+
 uint64_t tms_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char* tms_status_string(int status) {

@@ -72,22 +72,28 @@ topk_level_kernel(const float* __restrict__ scores, const uint64_t* __restrict__
 
 int64_t chunks_of(int64_t n) { return (n + CHUNK - 1) / CHUNK; }
 
-}  // namespace
+constexpr int MAX_SHARDS = 64;
+struct ShardBases { int64_t base[MAX_SHARDS]; };
 
-// two ping-pong key buffers, each sized for level 1's survivors
-size_t topk_workspace_bytes(int Q, int64_t B, int k) {
-    if (B <= CHUNK) return 0;
-    return 2 * sizeof(uint64_t) * (size_t)Q * (size_t)chunks_of(B) * (size_t)k;
+// keys[q, g*k_in + r] = key(values[g, q, r], shard_base[g] + indices[g, q, r]): the candidates of a k-way merge
+__global__ void merge_keys_kernel(const float* __restrict__ values, const int64_t* __restrict__ indices, int G, int Q,
+                                  int k_in, const ShardBases bases, uint64_t* __restrict__ keys) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t per_q = (int64_t)G * k_in;
+    if (i >= (int64_t)Q * per_q) return;
+    const int q = (int)(i / per_q);
+    const int64_t c = i - (int64_t)q * per_q;
+    const int g = (int)(c / k_in), r = (int)(c - (int64_t)g * k_in);
+    const int64_t src = ((int64_t)g * Q + q) * k_in + r;
+    keys[i] = make_key(values[src], (uint32_t)(bases.base[g] + indices[src]));
 }
 
-int launch_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
-                cudaStream_t stream) {
-    int64_t n = B;
-    const int64_t pitch1 = chunks_of(B) * k;  // keys per query in either buffer (level 1 is the largest)
-    uint64_t* buf[2] = {static_cast<uint64_t*>(workspace), static_cast<uint64_t*>(workspace) + (size_t)Q * pitch1};
+// runs the selection levels over keys_in[q, 0..n) (or scores when keys_in == nullptr) down to values / indices
+int run_levels(const float* scores, const uint64_t* keys_in, int64_t n, int64_t in_pitch, int Q, int k, uint64_t* buf0,
+               uint64_t* buf1, int64_t pitch1, float* values, int64_t* indices, cudaStream_t stream) {
+    uint64_t* buf[2] = {buf0, buf1};
     const float* s_in = scores;
-    const uint64_t* k_in = nullptr;
-    int64_t in_pitch = B;
+    const uint64_t* k_in = keys_in;
     int level = 0;
     while (true) {
         const int64_t nch = chunks_of(n);
@@ -105,6 +111,46 @@ int launch_topk(const float* scores, int Q, int64_t B, int k, float* values, int
         ++level;
     }
     return TMS_OK;
+}
+
+}  // namespace
+
+// two ping-pong key buffers, each sized for level 1's survivors
+size_t topk_workspace_bytes(int Q, int64_t B, int k) {
+    if (B <= CHUNK) return 0;
+    return 2 * sizeof(uint64_t) * (size_t)Q * (size_t)chunks_of(B) * (size_t)k;
+}
+
+int launch_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
+                cudaStream_t stream) {
+    const int64_t pitch1 = chunks_of(B) * k;  // keys per query in either buffer (level 1 is the largest)
+    uint64_t* b0 = static_cast<uint64_t*>(workspace);
+    return run_levels(scores, nullptr, B, B, Q, k, b0, b0 ? b0 + (size_t)Q * pitch1 : nullptr, pitch1, values, indices,
+                      stream);
+}
+
+// candidates [Q, G*k_in] followed by the two ping-pong buffers of the selection levels
+size_t topk_merge_workspace_bytes(int G, int Q, int k_in, int k) {
+    const int64_t n = (int64_t)G * k_in;
+    size_t bytes = sizeof(uint64_t) * (size_t)Q * (size_t)n;
+    if (n > CHUNK) bytes += 2 * sizeof(uint64_t) * (size_t)Q * (size_t)chunks_of(n) * (size_t)k;
+    return bytes;
+}
+
+int launch_topk_merge(const float* values, const int64_t* indices, const int64_t* shard_base, int G, int Q, int k_in,
+                      int k, float* out_values, int64_t* out_indices, void* workspace, cudaStream_t stream) {
+    if (G > MAX_SHARDS) return TMS_ERR_UNSUPPORTED;
+    ShardBases bases = {};
+    for (int g = 0; g < G; ++g) bases.base[g] = shard_base[g];
+    const int64_t n = (int64_t)G * k_in;
+    uint64_t* keys = static_cast<uint64_t*>(workspace);
+    const int64_t total = (int64_t)Q * n;
+    merge_keys_kernel<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(values, indices, G, Q, k_in, bases, keys);
+    count_launch();
+    if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+    const int64_t pitch1 = chunks_of(n) * k;
+    uint64_t* b0 = keys + (size_t)total;
+    return run_levels(nullptr, keys, n, n, Q, k, b0, b0 + (size_t)Q * pitch1, pitch1, out_values, out_indices, stream);
 }
 
 }  // namespace tms

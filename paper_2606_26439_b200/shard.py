@@ -78,3 +78,18 @@ def gather_scores(local_scores, world_size: int):
     for r in range(world_size):
         parts[r].copy_(bufs[r][:, :parts[r].shape[1]])
     return torch.cat(parts, dim=1)
+
+
+def rank_seed(seed: int, rank: int) -> int:
+    """Seed of rank `rank`'s synthetic shard in bench.py's weak-scaling runs (every rank owns its own B documents)."""
+    return int(seed) + 1000 * int(rank)
+
+
+def aggregate_throughput(units_per_rank: float, local_ms: float, device=None):
+    """(whole-job units/s, max-over-ranks ms): every rank processed `units_per_rank` units in `local_ms` of device time;
+    the job's time is the slowest rank's (bench.py's `value`; identity on one rank)."""
+    import torch.distributed as dist
+
+    world = dist.get_world_size() if dist.is_available() and dist.is_initialized() else 1
+    ms = max_over_ranks(local_ms, device)
+    return world * units_per_rank / (ms * 1e-3), ms

@@ -40,6 +40,8 @@ SIGNATURES = {
     "tms_pq_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i, _i, _i64]),
     "tms_topk": (_i, [_vp, _i, _i64, _i, _vp, _vp, _vp, _sz, _vp]),
     "tms_topk_workspace_bytes": (_sz, [_i, _i64, _i]),
+    "tms_topk_merge": (_i, [_vp, _vp, _vp, _i, _i, _i, _i, _vp, _vp, _vp, _sz, _vp]),
+    "tms_topk_merge_workspace_bytes": (_sz, [_i, _i, _i, _i]),
     "tms_launch_count": (_u64, []),
     "tms_status_string": (ctypes.c_char_p, [_i]),
     "tms_version": (_i, []),
@@ -276,3 +278,22 @@ def tms_pq_maxsim_decode_host(queries: torch.Tensor, codebooks: torch.Tensor, co
                                           dev_workspace.numel() * dev_workspace.element_size(), _stream(stream))
     _check(st, "tms_pq_maxsim_decode_host")
     return scores
+
+
+def tms_topk_merge(values: torch.Tensor, indices: torch.Tensor, shard_base, k: int, stream=None):
+    """k best of G per-shard top-k lists: values / indices [G,Q,k_in] (shard-local indices), shard_base[g] = first
+    global document of shard g.  Returns (values[Q,k], indices[Q,k]) with GLOBAL document indices."""
+    G, Q, k_in = values.shape
+    if values.dtype != torch.float32 or indices.dtype != torch.int64 or indices.shape != values.shape:
+        raise ValueError("values fp32 [G,Q,k_in] and indices int64 [G,Q,k_in] expected")
+    base = (ctypes.c_int64 * G)(*[int(b) for b in shard_base])
+    out_v = torch.empty((Q, k), dtype=torch.float32, device=values.device)
+    out_i = torch.empty((Q, k), dtype=torch.int64, device=values.device)
+    lib = load()
+    need = int(lib.tms_topk_merge_workspace_bytes(G, Q, k_in, k))
+    ws = torch.empty(max(need, 8), dtype=torch.uint8, device=values.device)
+    st = lib.tms_topk_merge(_dev(values, "values"), _dev(indices, "indices"), ctypes.addressof(base), G, Q, k_in, k,
+                            _dev(out_v, "out_values"), _dev(out_i, "out_indices"), _dev(ws, "workspace"), ws.numel(),
+                            _stream(stream))
+    _check(st, "tms_topk_merge")
+    return out_v, out_i

@@ -85,3 +85,65 @@ def test_two_ranks_score_their_shards_and_concatenate():
     for rank, ok, slowest, total in results:
         assert ok, f"rank {rank}: gathered scores differ from the single-process result"
         assert slowest == float(world) and total == float(len(lens))
+
+
+def _bench_rank_worker(rank, world, port, out):
+    """The rank logic of bench.py (shard.rank_seed, shard.aggregate_throughput) on two gloo processes."""
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        B = 1000
+        seed = shard.rank_seed(7, rank)
+        lens = synth.lognormal_lengths(B, seed=seed)  # every rank draws its own shard, as bench.py does
+        local_ms = 2.0 + 3.0 * rank                    # rank 1 is the slow one
+        value, ms = shard.aggregate_throughput(B, local_ms)
+        out.put((rank, seed, int(lens.sum()), value, ms))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(180)
+def test_bench_rank_logic_on_two_gloo_ranks():
+    world = 2
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_bench_rank_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    results = sorted(out.get(timeout=150) for _ in range(world))
+    for p in procs:
+        p.join(30)
+        assert p.exitcode == 0
+    (r0, s0, t0, v0, ms0), (r1, s1, t1, v1, ms1) = results
+    assert (s0, s1) == (7, 1007) and t0 != t1, "ranks must own different shards"
+    assert ms0 == ms1 == 5.0, "the job's time is the slowest rank's"
+    assert v0 == v1 == pytest.approx(2 * 1000 / 5.0e-3), "value is the whole-job aggregate"
+    assert shard.aggregate_throughput(1000, 4.0) == (pytest.approx(250000.0), 4.0)  # one process: identity
+
+
+def test_bench_gpus_flag_spawns_its_own_ranks():
+    """`python bench.py --gpus N` must start N ranks itself (no launcher): checked on the command it builds."""
+    import importlib.util
+    import sys
+    from unittest import mock
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    seen = {}
+
+    def fake_call(cmd, env=None):
+        seen["cmd"], seen["env"] = cmd, env
+        return 0
+
+    argv = ["bench.py", "--gpus", "4", "--steps", "2", "--warmup", "3"]
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    with mock.patch.object(sys, "argv", argv), mock.patch("subprocess.call", fake_call), \
+            mock.patch.dict(os.environ, env, clear=True), pytest.raises(SystemExit) as e:
+        bench.main()
+    assert e.value.code == 0
+    cmd = seen["cmd"]
+    assert "torch.distributed.run" in cmd and "--nproc-per-node=4" in cmd and "127.0.0.1" in cmd
+    assert cmd[-6:] == argv[1:] and "NCCL_DEBUG" in seen["env"]
