@@ -850,10 +850,18 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             // The codebook goes to shared memory once per CTA, already split: plane 0 holds every centroid slice's
             // eight bf16 hi parts (16 bytes per (m, k)), plane 1 the lo parts.  Decoding a token is then a pure gather:
             // token row r's 16 codes -> per 64-dimension unit, eight 16-byte hi pieces and eight lo pieces.
+            // Layout [m / 8][k][m % 8][16 bytes]: sub-quantiser m lives in bank group m % 8 whatever the code is.  At
+            // step oc thread r handles m % 8 = A(r % 8) ^ oc, A = multiplication by x in GF(8) (x^3 + x + 1): A and A + I
+            // are both bijections, so the eight lanes of a quarter-warp READ eight different bank groups (m % 8) and
+            // WRITE eight different ones (the operand swizzle puts piece m % 8 of row r into group (m % 8) ^ (r % 8)) --
+            // a random gather with no bank conflicts at all.
+            const uint32_t ar = ((sw << 1) ^ ((sw & 4u) ? 0xbu : 0u)) & 7u;  // A(r % 8)
             {
                 const uint4* g = reinterpret_cast<const uint4*>(p.codebooks);
-                for (int e = r; e < 16 * 256; e += 128) {
-                    const uint4 y0 = ldg_nc16(g + 2 * e), y1 = ldg_nc16(g + 2 * e + 1);
+                for (int e0 = r; e0 < 16 * 256; e0 += 128) {
+                    const int m_ = e0 >> 8, k_ = e0 & 255;
+                    const int e = (((m_ >> 3) * 256 + k_) << 3) + (m_ & 7);
+                    const uint4 y0 = ldg_nc16(g + 2 * e0), y1 = ldg_nc16(g + 2 * e0 + 1);
                     uint4 hi, lo;
                     split_pair(__uint_as_float(y0.x), __uint_as_float(y0.y), hi.x, lo.x);
                     split_pair(__uint_as_float(y0.z), __uint_as_float(y0.w), hi.y, lo.y);
@@ -872,13 +880,14 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
                     uint8_t* op = st_ptr + (size_t)s * stage_bytes + r * KB_BYTES;
 #pragma unroll
-                    for (int oc = 0; oc < 8; ++oc) {  // sub-quantiser m = 8*ch + oc fills 16-byte piece oc of the unit
-                        const uint32_t wsel = ch == 0 ? (oc < 4 ? cword[0] : cword[1]) : (oc < 4 ? cword[2] : cword[3]);
-                        const uint32_t code = (wsel >> (8 * (oc & 3))) & 0xffu;
-                        const uint8_t* e = cb_ptr + ((size_t)((8 * ch + oc) * 256 + code) << 4);
+                    for (int oc = 0; oc < 8; ++oc) {  // sub-quantiser m = 8*ch + mm fills 16-byte piece mm of the unit
+                        const uint32_t mm = ar ^ (uint32_t)oc;
+                        const uint32_t wsel = (mm & 4u) ? cword[2 * ch + 1] : cword[2 * ch];
+                        const uint32_t code = __byte_perm(wsel, 0u, 0x4440u | (mm & 3u));
+                        const uint8_t* e = cb_ptr + ((size_t)(((uint32_t)ch * 256u + code) * 8u + mm) << 4);
                         const uint4 hi = *reinterpret_cast<const uint4*>(e);
                         const uint4 lo = *reinterpret_cast<const uint4*>(e + cb_bytes / 2);
-                        const uint32_t o = ((uint32_t)oc ^ sw) << 4;
+                        const uint32_t o = (mm ^ sw) << 4;
                         *reinterpret_cast<uint4*>(op + o) = hi;
                         *reinterpret_cast<uint4*>(op + KB_TILE_BYTES + o) = lo;
                     }
