@@ -62,6 +62,8 @@ WORKLOADS = {
     # NEXT-4: the same scores as c5 from the decode-and-contract variant (codebook in shared memory, tensor cores)
     "c5-decode": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
                       decode=True),
+    "c5-decode-fp16": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16,
+                           K=256, decode=True, precision="fp16"),
     "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256),
 }
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
@@ -333,8 +335,9 @@ class Workload:
                 if variant == "auto" else variant
         elif w.get("decode"):
             def step():
-                tms.tms_pq_maxsim_decode(inp["q"], inp["C"], inp["store"], self.off_d, scores=self.scores)
-            self.kernel = "tcgen05 (decode-and-contract)"
+                tms.tms_pq_maxsim_decode(inp["q"], inp["C"], inp["store"], self.off_d, scores=self.scores,
+                                         precision=w.get("precision", "split_bf16"))
+            self.kernel = "tcgen05 (decode-and-contract, %s operands)" % w.get("precision", "split_bf16")
         else:
             lut = torch.empty((Q, Nq, w["M"], w["K"]), dtype=torch.float32, device=dev)
             ws = torch.empty(max(tms.tms_pq_workspace_bytes(Q, Nq, w["M"], w["K"], B), 16), dtype=torch.uint8, device=dev)
@@ -404,7 +407,7 @@ def roofline_of(wl, step_ms, total_ms, clocks, peaks):
         # tensor work: 2*Q*Nq*T*d algorithmic FLOP.  fp32 inputs cost three bf16 MMAs per product, the PQ
         # decode variant two (bf16 queries), so their tensor peaks are a third / half of the bf16 peak.
         fl = accounting.dense_flops(w["Q"], w["Nq"], w["d"], T)
-        div = 2.0 if w.get("decode") else (3.0 if w["dtype"] == "fp32" else 1.0)
+        div = (1.0 if w.get("precision") == "fp16" else 2.0) if w.get("decode") else (3.0 if w["dtype"] == "fp32" else 1.0)
         tfl = fl / kern_s / 1e12
         common["tensor"] = {"achieved_TFLOPs": tfl, "mma_per_product": div, "algorithmic_flops_per_launch": fl,
                             "peak_TFLOPs_burst": tc_burst / div, "frac_burst": tfl / (tc_burst / div),
@@ -445,7 +448,7 @@ def roofline_of(wl, step_ms, total_ms, clocks, peaks):
 
 
 SECONDARY = ["c2-q4", "c2-q1", "c2-fp16", "c2-fp32", "c3-100k", "c3-250k", "c3-500k", "c4-d64", "c4-d256", "c4-d512",
-             "c4-d768", "c5", "c5-decode"]
+             "c4-d768", "c5", "c5-decode", "c5-decode-fp16"]
 
 
 def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):

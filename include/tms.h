@@ -145,6 +145,20 @@ int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_
                          int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
                          float* scores, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Operand precision of tms_pq_maxsim_decode_variant. */
+typedef enum {
+    TMS_PQ_SPLIT_BF16 = 0, /* the default: bf16 hi + lo parts, two MMAs per product, ~1e-5 from the fp32 table form  */
+    TMS_PQ_FP16 = 1        /* queries and centroids rounded to fp16 (11-bit mantissa), ONE MMA per product: half the
+                              tensor work; per-element rounding 2^-12 relative, measured |dscore| <= 1e-3*Nq on config
+                              5's data (inside the 2e-3*Nq tolerance of 16-bit inputs); inputs must fit fp16's range  */
+} tms_pq_precision;
+
+/* tms_pq_maxsim_decode with an explicit operand precision (tms_pq_maxsim_decode = TMS_PQ_SPLIT_BF16). */
+int tms_pq_maxsim_decode_variant(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks,
+                                 int M, int K, const uint8_t* codes, const int64_t* offsets, int64_t B,
+                                 int64_t total_tokens, float* scores, void* workspace, size_t workspace_bytes,
+                                 void* stream, tms_pq_precision precision);
+
 /*
  * Host-buffer entry points: identical results, but `queries`, `docs` / `codes`, `offsets`, `codebooks` and
  * `scores` are HOST pointers (pinned memory makes the copies asynchronous and fast).  The document store

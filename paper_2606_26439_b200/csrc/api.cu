@@ -188,9 +188,11 @@ size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B) {
     return pq_smem_workspace_bytes(Q, Nq);
 }
 
-int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
-                         int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
-                         float* scores, void* workspace, size_t workspace_bytes, void* stream) {
+int tms_pq_maxsim_decode_variant(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks,
+                                 int M, int K, const uint8_t* codes, const int64_t* offsets, int64_t B,
+                                 int64_t total_tokens, float* scores, void* workspace, size_t workspace_bytes,
+                                 void* stream, tms_pq_precision precision) {
+    if (precision != TMS_PQ_SPLIT_BF16 && precision != TMS_PQ_FP16) return TMS_ERR_INVALID_ARG;
     if (Q <= 0 || Nq <= 0 || d <= 0 || M <= 0 || K <= 0 || B < 0 || total_tokens < 0) return TMS_ERR_INVALID_ARG;
     if (q_dtype != TMS_DTYPE_F32 && q_dtype != TMS_DTYPE_F16 && q_dtype != TMS_DTYPE_BF16) return TMS_ERR_INVALID_ARG;
     if (!queries || !codebooks || !offsets || (B > 0 && !scores) || (total_tokens > 0 && !codes))
@@ -211,7 +213,15 @@ int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_
                 workspace, workspace_bytes};
     a.codes = codes;
     a.codebooks = codebooks;
+    a.pq_half = precision == TMS_PQ_FP16;
     return dense_tc_supports(a) ? launch_dense_tc(a) : TMS_ERR_UNSUPPORTED;
+}
+
+int tms_pq_maxsim_decode(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
+                         int K, const uint8_t* codes, const int64_t* offsets, int64_t B, int64_t total_tokens,
+                         float* scores, void* workspace, size_t workspace_bytes, void* stream) {
+    return tms_pq_maxsim_decode_variant(queries, Q, Nq, d, q_dtype, codebooks, M, K, codes, offsets, B, total_tokens,
+                                        scores, workspace, workspace_bytes, stream, TMS_PQ_SPLIT_BF16);
 }
 
 int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,

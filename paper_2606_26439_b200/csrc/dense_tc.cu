@@ -68,6 +68,7 @@ struct Params {
     const float* codebooks;
     int q_fmt;             // element type of the query rows: 0 fp32, 1 fp16, 2 bf16 (fp32-split paths only)
     int skip_alo;          // the queries' lo halves are all zero (bf16 queries): leave out the a_lo * b_hi MMAs
+    int half_mode;         // PQD, TMS_PQ_FP16: queries and centroids rounded to fp16, one MMA per product (no lo parts)
 #ifdef TMS_PROBES
     const void* docs_raw;
     int debug;             // probe builds only (-DTMS_PROBES, never set by build.py): TMS_DEBUG bits 1 skip epilogue
@@ -246,6 +247,16 @@ __device__ __forceinline__ void split_pair(float x0, float x1, uint32_t& hi, uin
     const __nv_bfloat162 l = __floats2bfloat162_rn(x0 - hf.x, x1 - hf.y);
     hi = *reinterpret_cast<const uint32_t*>(&h);
     lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+// operand encoding of the split paths: bf16 hi/lo pair, or (half_mode) one fp16 value rounded to nearest even, lo = 0
+__device__ __forceinline__ void encode_pair(float x0, float x1, uint32_t& hi, uint32_t& lo, bool half_mode) {
+    if (half_mode) {
+        const __half2 h = __floats2half2_rn(x0, x1);
+        hi = *reinterpret_cast<const uint32_t*>(&h);
+        lo = 0u;
+    } else {
+        split_pair(x0, x1, hi, lo);
+    }
 }
 __device__ __forceinline__ uint4 ldg_nc16(const void* p) {
     uint4 r;
@@ -678,7 +689,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // descriptor is the previous one plus a constant); only the tcgen05 instructions sit in elect_one() regions.
         const uint32_t b_lo0 = ((smem_u32(st_ptr) & 0x3FFFFu) >> 4) | DESC_LO;
         const uint32_t idesc = p.idesc;
-        const bool skip = PROBE(p, 2), skip_alo = p.skip_alo != 0;
+        const bool skip = PROBE(p, 2), skip_alo = p.skip_alo != 0, skip_blo = PQD && p.half_mode != 0;
         const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS, nch = (uint32_t)nchunks;
         const uint32_t acc0 = tmem_base + (uint32_t)p.acc_col0;
         // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
@@ -735,7 +746,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                                     const uint64_t b_lw = ((uint64_t)DESC_HI << 32) | (b_lo + (KB_TILE_BYTES >> 4) + kk * 2);
                                     const uint32_t a_hi = a_col + mb * a_mb_step + kk * 8;
                                     tc_mma_ts(d_tmem, a_hi, b_hi, idesc, (ch != 0 || kk != 0) ? 1u : 0u);
-                                    tc_mma_ts(d_tmem, a_hi, b_lw, idesc, 1u);
+                                    if (!skip_blo) tc_mma_ts(d_tmem, a_hi, b_lw, idesc, 1u);
                                     if (!skip_alo) tc_mma_ts(d_tmem, a_hi + a_lo_off, b_hi, idesc, 1u);
                                 }
                             } else {
@@ -856,6 +867,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             // WRITE eight different ones (the operand swizzle puts piece m % 8 of row r into group (m % 8) ^ (r % 8)) --
             // a random gather with no bank conflicts at all.
             const uint32_t ar = ((sw << 1) ^ ((sw & 4u) ? 0xbu : 0u)) & 7u;  // A(r % 8)
+            const bool half_mode = p.half_mode != 0;
             {
                 const uint4* g = reinterpret_cast<const uint4*>(p.codebooks);
                 for (int e0 = r; e0 < 16 * 256; e0 += 128) {
@@ -863,10 +875,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     const int e = (((m_ >> 3) * 256 + k_) << 3) + (m_ & 7);
                     const uint4 y0 = ldg_nc16(g + 2 * e0), y1 = ldg_nc16(g + 2 * e0 + 1);
                     uint4 hi, lo;
-                    split_pair(__uint_as_float(y0.x), __uint_as_float(y0.y), hi.x, lo.x);
-                    split_pair(__uint_as_float(y0.z), __uint_as_float(y0.w), hi.y, lo.y);
-                    split_pair(__uint_as_float(y1.x), __uint_as_float(y1.y), hi.z, lo.z);
-                    split_pair(__uint_as_float(y1.z), __uint_as_float(y1.w), hi.w, lo.w);
+                    encode_pair(__uint_as_float(y0.x), __uint_as_float(y0.y), hi.x, lo.x, half_mode);
+                    encode_pair(__uint_as_float(y0.z), __uint_as_float(y0.w), hi.y, lo.y, half_mode);
+                    encode_pair(__uint_as_float(y1.x), __uint_as_float(y1.y), hi.z, lo.z, half_mode);
+                    encode_pair(__uint_as_float(y1.z), __uint_as_float(y1.w), hi.w, lo.w, half_mode);
                     *reinterpret_cast<uint4*>(cb_ptr + e * 16) = hi;
                     *reinterpret_cast<uint4*>(cb_ptr + cb_bytes / 2 + e * 16) = lo;
                 }
@@ -885,11 +897,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         const uint32_t wsel = (mm & 4u) ? cword[2 * ch + 1] : cword[2 * ch];
                         const uint32_t code = __byte_perm(wsel, 0u, 0x4440u | (mm & 3u));
                         const uint8_t* e = cb_ptr + ((size_t)(((uint32_t)ch * 256u + code) * 8u + mm) << 4);
-                        const uint4 hi = *reinterpret_cast<const uint4*>(e);
-                        const uint4 lo = *reinterpret_cast<const uint4*>(e + cb_bytes / 2);
                         const uint32_t o = (mm ^ sw) << 4;
-                        *reinterpret_cast<uint4*>(op + o) = hi;
-                        *reinterpret_cast<uint4*>(op + KB_TILE_BYTES + o) = lo;
+                        *reinterpret_cast<uint4*>(op + o) = *reinterpret_cast<const uint4*>(e);
+                        if (!half_mode)
+                            *reinterpret_cast<uint4*>(op + KB_TILE_BYTES + o) = *reinterpret_cast<const uint4*>(e + cb_bytes / 2);
                     }
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     __syncwarp();
@@ -945,6 +956,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         if (set == 0)
         {
             const bool row_valid = (q < p.Q) && (i < p.Nq);
+            const bool half_mode = PQD && p.half_mode != 0;
             const uint8_t* src = static_cast<const uint8_t*>(p.queries) + ((int64_t)q * p.Nq + i) * p.row_bytes;
             for (int kb = 0; kb < p.NKB; ++kb) {
                 if constexpr (F32) {
@@ -956,8 +968,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                             for (int j = 0; j < 8; ++j) {
                                 uint4 x = make_uint4(0, 0, 0, 0);
                                 if (row_valid) x = ldg_nc16(src + kb * 256 + half * 128 + j * 16);
-                                split_pair(__uint_as_float(x.x), __uint_as_float(x.y), hi[2 * j], lo[2 * j]);
-                                split_pair(__uint_as_float(x.z), __uint_as_float(x.w), hi[2 * j + 1], lo[2 * j + 1]);
+                                encode_pair(__uint_as_float(x.x), __uint_as_float(x.y), hi[2 * j], lo[2 * j], half_mode);
+                                encode_pair(__uint_as_float(x.z), __uint_as_float(x.w), hi[2 * j + 1], lo[2 * j + 1], half_mode);
                             }
                         } else {             // 16-bit query rows (PQD): widened exactly to fp32 first
 #pragma unroll
@@ -976,7 +988,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                                         f0 = f.x;
                                         f1 = f.y;
                                     }
-                                    split_pair(f0, f1, hi[4 * j + e], lo[4 * j + e]);
+                                    encode_pair(f0, f1, hi[4 * j + e], lo[4 * j + e], half_mode);
                                 }
                             }
                         }
@@ -1255,7 +1267,8 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.codes = a.codes;
     p.codebooks = a.codebooks;
     p.q_fmt = (int)a.dtype;  // tms_dtype: 0 fp32, 1 fp16, 2 bf16
-    p.skip_alo = pqd && a.dtype == TMS_DTYPE_BF16;  // bf16 queries split into (x, 0)
+    p.half_mode = pqd && a.pq_half;
+    p.skip_alo = pqd && (a.dtype == TMS_DTYPE_BF16 || a.pq_half);  // bf16 queries split into (x, 0); fp16 mode has no lo parts
     p.NACC = (TMEM_COLS - MB * a_cols_per_block) / BN;
     if (p.NACC > MAX_ACC) p.NACC = MAX_ACC;
     p.acc_col0 = TMEM_COLS - p.NACC * BN;
@@ -1266,7 +1279,7 @@ bool plan(const DenseArgs& a, Plan& pl) {
         p.docs_raw = a.docs;
     }
 #endif
-    const uint32_t fmt = (!f32 && a.dtype == TMS_DTYPE_F16) ? 0u : 1u;  // the split paths feed bf16 pairs
+    const uint32_t fmt = ((!f32 && a.dtype == TMS_DTYPE_F16) || (pqd && a.pq_half)) ? 0u : 1u;  // the split paths feed bf16 pairs
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     pl.MB = MB;

@@ -38,6 +38,7 @@ struct DenseArgs {
     // queries' dtype and d = 128
     const uint8_t* codes = nullptr;
     const float* codebooks = nullptr;
+    bool pq_half = false;  // TMS_PQ_FP16: queries and centroids rounded to fp16, one MMA per product
 };
 
 // CUDA-core tiled kernel: any dtype / d / Nq / Q (csrc/dense_simt.cu).

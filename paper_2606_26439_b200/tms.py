@@ -32,6 +32,7 @@ SIGNATURES = {
     "tms_pq_maxsim_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
     "tms_pq_workspace_bytes": (_sz, [_i, _i, _i, _i, _i64]),
     "tms_pq_maxsim_decode": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
+    "tms_pq_maxsim_decode_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
     "tms_maxsim_host": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_decode_host": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
@@ -172,9 +173,12 @@ def tms_pq_maxsim(lut: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor,
     return scores
 
 
+PQ_PRECISIONS = {"split_bf16": 0, "fp16": 1}
+
+
 def tms_pq_maxsim_decode(queries: torch.Tensor, codebooks: torch.Tensor, codes: torch.Tensor, offsets: torch.Tensor,
                          scores: torch.Tensor | None = None, workspace: torch.Tensor | None = None,
-                         stream=None) -> torch.Tensor:
+                         stream=None, precision: str = "split_bf16") -> torch.Tensor:
     """Same value as tms_pq_build_lut + tms_pq_maxsim, decoded tile by tile in shared memory and contracted on the
     tensor cores (include/tms.h: tms_pq_maxsim_decode)."""
     Q, Nq, d = queries.shape
@@ -190,10 +194,10 @@ def tms_pq_maxsim_decode(queries: torch.Tensor, codebooks: torch.Tensor, codes: 
         workspace = torch.empty(need, dtype=torch.uint8, device=queries.device)
     ws_ptr = _dev(workspace, "workspace") if workspace is not None else None
     ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
-    st = lib.tms_pq_maxsim_decode(_dev(queries, "queries"), Q, Nq, d, _DTYPES[queries.dtype],
-                                  _dev(codebooks, "codebooks"), M, K, _dev(codes, "codes") if T else None,
-                                  _dev(offsets, "offsets"), B, T, _dev(scores, "scores") if B else None, ws_ptr, ws_len,
-                                  _stream(stream))
+    st = lib.tms_pq_maxsim_decode_variant(_dev(queries, "queries"), Q, Nq, d, _DTYPES[queries.dtype],
+                                          _dev(codebooks, "codebooks"), M, K, _dev(codes, "codes") if T else None,
+                                          _dev(offsets, "offsets"), B, T, _dev(scores, "scores") if B else None, ws_ptr,
+                                          ws_len, _stream(stream), PQ_PRECISIONS[precision])
     _check(st, "tms_pq_maxsim_decode")
     return scores
 

@@ -139,3 +139,27 @@ def test_decode_variant_rejects_other_shapes():
     q, C, codes = pq_case(1, 8, 8, 64, 4, off, seed=1)
     with pytest.raises(RuntimeError, match="unsupported"):
         tms.tms_pq_maxsim_decode(q.to(DEV), C.to(DEV), codes.to(DEV), torch.from_numpy(off).to(DEV))
+
+
+def test_decode_fp16_operands_within_the_16_bit_tolerance():
+    """TMS_PQ_FP16: queries and centroids rounded to fp16, one MMA per product.  Must stay inside 2e-3*Nq of the oracle
+    (which decompresses the fp32 codebooks exactly), and much closer in practice; exact on integer codebooks."""
+    lens = np.concatenate([[5, 128, 1, 0, 300, 127, 129, 64, 0, 17], synth.lognormal_lengths(3000, seed=11)])
+    off = synth.offsets_from_lengths(lens)
+    Q, Nq, T = 8, 32, int(off[-1])
+    q = synth.unit_tokens(Q * Nq, 128, torch.bfloat16, seed=51).view(Q, Nq, 128)
+    C = synth.pq_codebooks(16, 256, 8, seed=52)
+    codes = synth.pq_codes(T, 16, seed=53)
+    ref = oracle.pq_maxsim(q, C, codes, off)
+    od = torch.from_numpy(off).to(DEV)
+    got = tms.tms_pq_maxsim_decode(q.to(DEV), C.to(DEV), codes.to(DEV), od, precision="fp16").cpu().numpy().astype(np.float64)
+    inf = np.isneginf(ref)
+    assert np.array_equal(np.isneginf(got), inf)
+    err = np.abs(got[~inf] - ref[~inf]).max()
+    assert err <= 1e-3 * Nq, f"max |dscore| = {err:.3e}"
+    # integer queries and centroids are exact in fp16: bit-exact scores
+    qi = synth.small_int_tokens(Q * Nq, 128, torch.float16, seed=54).view(Q, Nq, 128)
+    Ci = synth.small_int_tokens(16 * 256, 8, torch.float32, seed=55).view(16, 256, 8)
+    refi = oracle.pq_maxsim(qi, Ci, codes, off)
+    goti = tms.tms_pq_maxsim_decode(qi.to(DEV), Ci.to(DEV), codes.to(DEV), od, precision="fp16").cpu().numpy().astype(np.float64)
+    assert np.array_equal(goti, refi)
