@@ -64,7 +64,12 @@ WORKLOADS = {
                       decode=True),
     "c5-decode-fp16": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16,
                            K=256, decode=True, precision="fp16"),
-    "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256),
+    # configs[4] through tms_pq_maxsim as a caller gets it (TMS_VARIANT_AUTO: fp16 table entries in shared memory)
+    "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
+               pq_variant="pq_smem_f16"),
+    # the same LUT kernel over fp32 table entries (SURVEY 7.3 H6's A/B: twice the shared-memory gather bytes)
+    "c5-f32": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
+                   pq_variant="pq_smem"),
 }
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
 ELEM_BYTES = {"bf16": 2, "fp16": 2, "fp32": 4}
@@ -342,10 +347,15 @@ class Workload:
             lut = torch.empty((Q, Nq, w["M"], w["K"]), dtype=torch.float32, device=dev)
             ws = torch.empty(max(tms.tms_pq_workspace_bytes(Q, Nq, w["M"], w["K"], B), 16), dtype=torch.uint8, device=dev)
 
+            # "c5" calls with variant "auto"; its `pq_variant` names what AUTO runs for that shape (roofline bytes per
+            # entry); "c5-f32" forces the fp32-entry kernel
+            pq_variant = variant if (variant != "auto" or name == "c5") else w.get("pq_variant", "auto")
+
             def step():
                 tms.tms_pq_build_lut(inp["q"], inp["C"], lut=lut)
-                tms.tms_pq_maxsim(lut, inp["store"], self.off_d, scores=self.scores, workspace=ws, variant=variant)
-            self.kernel = "pq_smem" if ws.numel() > 16 else "pq_simt"
+                tms.tms_pq_maxsim(lut, inp["store"], self.off_d, scores=self.scores, workspace=ws, variant=pq_variant)
+            self.kernel = w.get("pq_variant", "pq_smem") if pq_variant == "auto" else pq_variant
+            self.entry_bytes = 2 if self.kernel == "pq_smem_f16" else 4
         self.step = step
 
 
@@ -426,10 +436,11 @@ def roofline_of(wl, step_ms, total_ms, clocks, peaks):
         # fused PQ (LUT form): Q*Nq*T*M four-byte shared-memory gathers against M bytes of codes per token -- bound by
         # the shared-memory load pipe (128 B/clk/SM), not by HBM and not by tensor cores
         lookups = accounting.pq_lookups(w["Q"], w["Nq"], w["M"], T)
-        g = lookups * 4 / kern_s / 1e9
+        entry_bytes = wl.entry_bytes
+        g = lookups * entry_bytes / kern_s / 1e9
         roofline = {"bound": "alu", "achieved": g, "peak": SMEM_PIPE_PEAK_GBS, "unit": "GB/s", "frac": g / SMEM_PIPE_PEAK_GBS}
-        notes.append("shared-memory gather bytes/s against 148 SMs x 128 B/clk x 1.965 GHz; step = LUT build + relayout + "
-                     "fused lookup kernel")
+        notes.append("shared-memory gather bytes/s (%d-byte table entries) against 148 SMs x 128 B/clk x 1.965 GHz; step = "
+                     "LUT build + relayout + fused lookup kernel" % entry_bytes)
     # what THIS run observed about clocks and power (NVML samples taken while the timed steps ran)
     p_w, p_lim = clocks.get("power_w_mean"), clocks.get("power_limit_w")
     obs = "this run: NVML SM clock median %s MHz (max %s), throttle reasons %s" % (
@@ -448,7 +459,7 @@ def roofline_of(wl, step_ms, total_ms, clocks, peaks):
 
 
 SECONDARY = ["c2-q4", "c2-q1", "c2-fp16", "c2-fp32", "c3-100k", "c3-250k", "c3-500k", "c4-d64", "c4-d256", "c4-d512",
-             "c4-d768", "c5", "c5-decode", "c5-decode-fp16"]
+             "c4-d768", "c5", "c5-f32", "c5-decode", "c5-decode-fp16"]
 
 
 def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):

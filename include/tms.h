@@ -58,7 +58,9 @@ typedef enum {
     TMS_VARIANT_AUTO = 0,     /* what tms_maxsim / tms_pq_maxsim pick                                  */
     TMS_VARIANT_SIMT = 1,     /* CUDA-core tiled kernel: any dtype, any d, any Nq (the general path)   */
     TMS_VARIANT_TCGEN05 = 2,  /* TMA + tcgen05 tensor-core kernel (sm_100a), dimension-tiled for d>128 */
-    TMS_VARIANT_PQ_SMEM = 3   /* PQ: LUT slices resident in shared memory                              */
+    TMS_VARIANT_PQ_SMEM = 3,  /* PQ: LUT slices resident in shared memory                              */
+    TMS_VARIANT_PQ_SMEM_F16 = 4 /* PQ: the same with table entries held as (block-scaled) fp16 in shared memory:
+                                 half the gather bytes; see tms_pq_maxsim                                */
 } tms_variant;
 
 /*
@@ -119,6 +121,14 @@ int tms_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtyp
  * The decompressed vectors are never materialised.  The sum over m is fp32 in a fixed, kernel-defined
  * order (run-to-run reproducible).
  * workspace  device scratch of at least tms_pq_workspace_bytes(...) bytes (the re-laid-out table).
+ * Kernels: for M = 16, K = 256 the table is re-laid-out into the workspace and served from shared memory in slices
+ * (P:L268 keeps it in L2; here the gathers are the bound).  With Nq % 16 == 0 the re-laid-out copy holds the entries
+ * as fp16 after one power-of-two scale of the whole table (max|entry| -> [2^14, 2^15): no overflow or subnormals for
+ * any finite table), they are widened back inside the fp32 additions, and the scale is undone exactly: half the
+ * gather bytes, one rounding of relative 2^-11 per entry (measured max |dscore| on config 4's data: see DESIGN.md
+ * 5.4; tests hold it to a quarter of the 2e-3*Nq tolerance).  TMS_VARIANT_PQ_SMEM forces fp32 entries (Nq % 8 == 0),
+ * TMS_VARIANT_PQ_SMEM_F16 the fp16 ones, TMS_VARIANT_SIMT the general kernel (any M, K <= 256, Nq; table read
+ * through L1/L2).  `lut` itself is never modified.
  */
 int tms_pq_maxsim(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes, const int64_t* offsets,
                   int64_t B, int64_t total_tokens, float* scores, void* workspace, size_t workspace_bytes,

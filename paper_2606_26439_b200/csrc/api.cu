@@ -112,14 +112,20 @@ static int pq_dispatch(const float* lut, int Q, int Nq, int M, int K, const uint
     if (st != TMS_OK) return st;
     if (!device_info()) return TMS_ERR_CUDA;
     if (B == 0) return TMS_OK;
+    if (variant != TMS_VARIANT_AUTO && variant != TMS_VARIANT_SIMT && variant != TMS_VARIANT_PQ_SMEM &&
+        variant != TMS_VARIANT_PQ_SMEM_F16)
+        return TMS_ERR_INVALID_ARG;
+    // AUTO: the shared-memory kernel over fp16 table entries when the shape has whole 16-row slices (half the gather
+    // bytes, 1.9x faster on config 4, error well inside the 16-bit tolerance: DESIGN.md 5.4), else over fp32 entries
+    // (8-row slices), else the general kernel.  TMS_VARIANT_PQ_SMEM always means fp32 entries.
     PqArgs a{lut, Q, Nq, M, K, codes, offsets, B, T, scores, static_cast<cudaStream_t>(stream)};
-    const bool smem_ok = pq_smem_supports(a);
+    const bool f16 = variant == TMS_VARIANT_PQ_SMEM_F16 || (variant == TMS_VARIANT_AUTO && pq_smem_supports(a, true));
+    const bool smem_ok = pq_smem_supports(a, f16);
     if (variant == TMS_VARIANT_SIMT || (variant == TMS_VARIANT_AUTO && !smem_ok)) return launch_pq_simt(a);
-    if (variant != TMS_VARIANT_AUTO && variant != TMS_VARIANT_PQ_SMEM) return TMS_ERR_INVALID_ARG;
     if (!smem_ok) return TMS_ERR_UNSUPPORTED;
     if (!workspace || workspace_bytes < pq_smem_workspace_bytes(Q, Nq) || !aligned16(workspace))
         return TMS_ERR_WORKSPACE;
-    return launch_pq_smem(a, workspace);
+    return launch_pq_smem(a, workspace, f16);
 }
 
 }  // namespace tms

@@ -179,7 +179,7 @@ int tms_maxsim_host(const void* queries, int Q, int Nq, int d, const void* docs,
 size_t tms_pq_maxsim_host_workspace_min_bytes(int Q, int Nq, int d, tms_dtype q_dtype, int M, int K,
                                               int64_t max_doc_tokens) {
     if (Q <= 0 || Nq <= 0 || d <= 0 || M <= 0 || K <= 0 || max_doc_tokens < 0) return 0;
-    const size_t lut = up((size_t)Q * Nq * M * K * 4);
+    const size_t lut = up((size_t)Q * Nq * M * K * 4 + 16);  // the table, and the re-laid-out table + its header
     return up((size_t)Q * Nq * d * dtype_size(q_dtype)) + up((size_t)M * K * (d / M) * 4) + 2 * lut +
            2 * chunk_bytes(max_doc_tokens, 1, (size_t)M, Q, 0) + 2 * ALIGN;
 }
@@ -200,7 +200,7 @@ int tms_pq_maxsim_host(const void* queries, int Q, int Nq, int d, tms_dtype q_dt
     const size_t skew = (ALIGN - (reinterpret_cast<uintptr_t>(ws) % ALIGN)) % ALIGN;
     const size_t qbytes = up((size_t)Q * Nq * d * dtype_size(q_dtype));
     const size_t cbytes = up((size_t)M * K * (d / M) * 4);
-    const size_t lbytes = up((size_t)Q * Nq * M * K * 4);
+    const size_t lbytes = up((size_t)Q * Nq * M * K * 4 + 16);  // the table, and the re-laid-out table + its header
     const size_t fixed = skew + qbytes + cbytes + 2 * lbytes;
     if (dev_workspace_bytes < fixed + 4 * ALIGN) return TMS_ERR_WORKSPACE;
     uint8_t* q_dev = ws + skew;

@@ -91,9 +91,16 @@ pq_simt_kernel(const float* __restrict__ lut, int Q, int Nq, int M, int K, const
 // then read 16-byte pieces 2*((s+u)&3) + h of their (code-dependent) lines -- eight distinct bank groups,
 // conflict-free for any codes.  The per-lane order of the 16 additions is a fixed rotation of m.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int PQS_M = 16, PQS_K = 256, PQS_ROWS = 8;
-constexpr int PQS_SLICE_FLOATS = PQS_ROWS * PQS_M * PQS_K;  // 32768 floats = 128 KB
-constexpr int PQS_SLICE_BYTES = PQS_SLICE_FLOATS * 4;
+//
+// H16 (TMS_VARIANT_PQ_SMEM_F16): the same kernel over a table whose entries are stored as fp16 --
+// a slice is then 16 query rows, every LDS.128 returns eight rows' entries and the gather bytes (the bound of this
+// path) halve.  Entries are widened back to fp32 inside the addition (add.f32.f16: one FHADD per entry, as many ALU
+// instructions as the fp32 table needs), so only the STORED entry is rounded: one relative 2^-11 error per entry,
+// against the table's largest magnitude at worst, because the whole table is first scaled by a power of two that
+// brings max|entry| into [2^14, 2^15) (no overflow, no subnormals for any finite table; the scale is undone exactly
+// on the 16-row partial sums).
+constexpr int PQS_M = 16, PQS_K = 256;
+constexpr int PQS_SLICE_BYTES = 8 * PQS_M * PQS_K * 4;  // 128 KB: 8 rows of fp32 entries or 16 rows of fp16 entries
 constexpr int PQS_WARPS = 24, PQS_THREADS = PQS_WARPS * 32;
 constexpr int PQS_MAX_SC_FLOATS = 20480;  // 80 KB of per-chunk score accumulators
 
@@ -104,6 +111,34 @@ __global__ void pq_relayout_kernel(const float* __restrict__ lut, float* __restr
     const int row = (int)(o & 7), sub = (int)((o >> 3) & 3), k = (int)((o >> 5) & 255), g = (int)((o >> 13) & 3);
     const int64_t sl = o >> 15;
     lutT[o] = lut[((sl * 8 + row) * PQS_M + (4 * g + sub)) * PQS_K + k];
+}
+
+// max |lut| as float bits (non-negative floats order like unsigned integers); *out zeroed beforehand
+__global__ void pq_absmax_kernel(const float* __restrict__ lut, int64_t total, uint32_t* __restrict__ out) {
+    uint32_t m = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint32_t b = __float_as_uint(lut[i]) & 0x7fffffffu;
+        m = b > m ? b : m;
+    }
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0) atomicMax(out, m);
+}
+
+// lut [R, 16, 256] fp32 -> lutT [R/16 slices][4 g][256 k][4 sub][16 rows] fp16, scaled by the power of two that puts
+// max|lut| into [2^14, 2^15); hdr[0] = max|lut| bits (input), hdr[1] = 1/scale as float bits (output).
+__global__ void pq_relayout_f16_kernel(const float* __restrict__ lut, __half* __restrict__ lutT, int64_t total,
+                                       uint32_t* __restrict__ hdr) {
+    const float mx = __uint_as_float(hdr[0]);
+    int e = 15;
+    if (mx > 0.f && mx < INFINITY) frexpf(mx, &e);  // mx = f * 2^e, f in [0.5, 1)
+    const float scale = ldexpf(1.f, 15 - e);        // 15 - e in [-113, 164]: clamp so that the scale stays finite
+    const float sc = (15 - e > 126) ? ldexpf(1.f, 126) : scale;
+    const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o == 0) hdr[1] = __float_as_uint(1.f / sc);  // exact: a power of two
+    if (o >= total) return;
+    const int row = (int)(o & 15), sub = (int)((o >> 4) & 3), k = (int)((o >> 6) & 255), g = (int)((o >> 14) & 3);
+    const int64_t sl = o >> 16;
+    lutT[o] = __float2half_rn(lut[((sl * 16 + row) * PQS_M + (4 * g + sub)) * PQS_K + k] * sc);
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -133,11 +168,23 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ uint4 lds128u(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+// a += lo half of w, b += hi half of w, both widened exactly to fp32 inside the addition (one FHADD each)
+__device__ __forceinline__ void add_h2(float& a, float& b, uint32_t w) {
+    asm("add.rn.f32.f16 %0, %1, %0;" : "+f"(a) : "h"((unsigned short)(w & 0xffffu)));
+    asm("add.rn.f32.f16 %0, %1, %0;" : "+f"(b) : "h"((unsigned short)(w >> 16)));
+}
 
+template <bool H16>
 __global__ void __launch_bounds__(PQS_THREADS, 1)
-pq_smem_kernel(const float* __restrict__ lutT, int Q, int Nq, const uint8_t* __restrict__ codes,
+pq_smem_kernel(const void* __restrict__ lutT, int Q, int Nq, const uint8_t* __restrict__ codes,
                const int64_t* __restrict__ offsets, int64_t B, int dpc /* docs per chunk */, int64_t nchunks,
-               float* __restrict__ scores) {
+               float* __restrict__ scores, const float* __restrict__ inv_scale) {
+    constexpr int PQS_ROWS = H16 ? 16 : 8;  // query rows per 128 KB slice
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* lut_s = reinterpret_cast<float*>(smem_raw);                          // 128 KB slice
     float* sc = reinterpret_cast<float*>(smem_raw + PQS_SLICE_BYTES);           // [Q][dpc]
@@ -163,6 +210,7 @@ pq_smem_kernel(const float* __restrict__ lutT, int Q, int Nq, const uint8_t* __r
         base[s] = lut_a + sub * 32u + (uint32_t)h * 16u;
     }
     uint32_t phase = 0;
+    const float unscale = H16 ? *inv_scale : 1.f;
     __syncthreads();
 
     for (int64_t chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
@@ -175,13 +223,13 @@ pq_smem_kernel(const float* __restrict__ lutT, int Q, int Nq, const uint8_t* __r
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a),
                              "r"((uint32_t)PQS_SLICE_BYTES)
                              : "memory");
-                const float* src = lutT + (int64_t)sl * PQS_SLICE_FLOATS;
+                const uint8_t* src = static_cast<const uint8_t*>(lutT) + (int64_t)sl * PQS_SLICE_BYTES;
 #pragma unroll
                 for (int p = 0; p < 4; ++p)
                     asm volatile(
                         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
                             lut_a + p * (PQS_SLICE_BYTES / 4)),
-                        "l"(src + p * (PQS_SLICE_FLOATS / 4)), "r"((uint32_t)(PQS_SLICE_BYTES / 4)), "r"(bar_a)
+                        "l"(src + p * (PQS_SLICE_BYTES / 4)), "r"((uint32_t)(PQS_SLICE_BYTES / 4)), "r"(bar_a)
                         : "memory");
             }
             mbar_wait(bar_a, phase);
@@ -193,9 +241,47 @@ pq_smem_kernel(const float* __restrict__ lutT, int Q, int Nq, const uint8_t* __r
                 const int64_t t0 = offsets[d0 + dd];
                 const int n = (int)(offsets[d0 + dd + 1] - t0);
                 const uint8_t* cp = codes + (t0 + slot) * PQS_M;
-                float r0 = -INFINITY, r1 = -INFINITY, r2 = -INFINITY, r3 = -INFINITY;
+                float part;
                 uint4 c = make_uint4(0, 0, 0, 0);
                 if (slot < n) c = ldg_codes(cp);
+                if constexpr (H16) {
+                    float r[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) r[j] = -INFINITY;
+                    for (int tb = 0; tb < n; tb += 16) {
+                        uint4 cn = make_uint4(0, 0, 0, 0);
+                        if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M);  // prefetch next step
+                        float a[8];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) a[j] = 0.f;
+                        const uint32_t w[4] = {c.x, c.y, c.z, c.w};
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) {
+#pragma unroll
+                            for (int s = 0; s < 4; ++s) {
+                                const uint32_t code = __byte_perm(w[g], 0u, sel[s]);
+                                const uint4 v = lds128u(base[s] + code * 128u + (uint32_t)g * (PQS_K * 128u));
+                                add_h2(a[0], a[1], v.x); add_h2(a[2], a[3], v.y);
+                                add_h2(a[4], a[5], v.z); add_h2(a[6], a[7], v.w);
+                            }
+                        }
+                        if (tb + slot < n) {
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) r[j] = fmaxf(r[j], a[j]);
+                        }
+                        c = cn;
+                    }
+                    // max over the 16 token slots (lane bits 1..4), then sum of the 16 rows (8 here, 8 in lane ^ 1)
+#pragma unroll
+                    for (int o = 2; o <= 16; o <<= 1) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) r[j] = fmaxf(r[j], __shfl_xor_sync(0xffffffffu, r[j], o));
+                    }
+                    part = ((r[0] + r[1]) + (r[2] + r[3])) + ((r[4] + r[5]) + (r[6] + r[7]));
+                    part += __shfl_xor_sync(0xffffffffu, part, 1);
+                    part *= unscale;  // exact: a power of two
+                } else {
+                float r0 = -INFINITY, r1 = -INFINITY, r2 = -INFINITY, r3 = -INFINITY;
                 for (int tb = 0; tb < n; tb += 16) {
                     uint4 cn = make_uint4(0, 0, 0, 0);
                     if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M);  // prefetch next step
@@ -223,8 +309,9 @@ pq_smem_kernel(const float* __restrict__ lutT, int Q, int Nq, const uint8_t* __r
                     r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
                     r3 = fmaxf(r3, __shfl_xor_sync(0xffffffffu, r3, o));
                 }
-                float part = (r0 + r1) + (r2 + r3);
+                part = (r0 + r1) + (r2 + r3);
                 part += __shfl_xor_sync(0xffffffffu, part, 1);
+                }
                 if (lane == 0) {
                     float* dst = sc + q * dpc + dd;
                     *dst = first ? part : (*dst + part);
@@ -280,23 +367,15 @@ int launch_pq_simt(const PqArgs& a) {
     return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
 }
 
-bool pq_smem_supports(const PqArgs& a) {
-    return a.M == PQS_M && a.K == PQS_K && a.Nq % PQS_ROWS == 0 && a.Q >= 1 && a.Q <= PQS_MAX_SC_FLOATS / 16;
+bool pq_smem_supports(const PqArgs& a, bool f16) {
+    return a.M == PQS_M && a.K == PQS_K && a.Nq % (f16 ? 16 : 8) == 0 && a.Q >= 1 && a.Q <= PQS_MAX_SC_FLOATS / 16;
 }
 
-size_t pq_smem_workspace_bytes(int Q, int Nq) { return sizeof(float) * (size_t)Q * Nq * PQS_M * PQS_K; }
+// the re-laid-out table (fp32 entries: as large as lut; fp16 entries: half of it) + a 16-byte header (fp16: max, 1/scale)
+size_t pq_smem_workspace_bytes(int Q, int Nq) { return sizeof(float) * (size_t)Q * Nq * PQS_M * PQS_K + 16; }
 
-// workspace: the re-laid-out table lutT, same size as lut.
-int launch_pq_smem(const PqArgs& a, void* workspace) {
-    const DeviceInfo* di = device_info();
-    if (!di) return TMS_ERR_CUDA;
-    if (a.B == 0) return TMS_OK;
-    float* lutT = static_cast<float*>(workspace);
-    const int64_t total = (int64_t)a.Q * a.Nq * PQS_M * PQS_K;
-    pq_relayout_kernel<<<(unsigned)((total + 255) / 256), 256, 0, a.stream>>>(a.lut, lutT, total);
-    count_launch();
-    if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
-
+template <bool H16>
+static int launch_pq_smem_t(const PqArgs& a, const void* lutT, const float* inv_scale, const DeviceInfo* di) {
     // docs per chunk: as large as the smem score accumulators allow (amortises the 128 KB slice reloads),
     // but no larger than one CTA's share of a small batch
     int dpc_max = PQS_MAX_SC_FLOATS / a.Q;
@@ -306,13 +385,38 @@ int launch_pq_smem(const PqArgs& a, void* workspace) {
     if (dpc > dpc_max) dpc = dpc_max;
     const int64_t nchunks = (a.B + dpc - 1) / dpc;
     const size_t smem = (size_t)PQS_SLICE_BYTES + sizeof(float) * PQS_MAX_SC_FLOATS + 16;
-    if (cudaFuncSetAttribute(pq_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    if (cudaFuncSetAttribute(pq_smem_kernel<H16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return TMS_ERR_CUDA;
     const int64_t grid = nchunks < di->num_sms ? nchunks : di->num_sms;
-    pq_smem_kernel<<<(unsigned)grid, PQS_THREADS, smem, a.stream>>>(lutT, a.Q, a.Nq, a.codes, a.offsets, a.B,
-                                                                    (int)dpc, nchunks, a.scores);
+    pq_smem_kernel<H16><<<(unsigned)grid, PQS_THREADS, smem, a.stream>>>(lutT, a.Q, a.Nq, a.codes, a.offsets, a.B,
+                                                                         (int)dpc, nchunks, a.scores, inv_scale);
     count_launch();
     return cudaGetLastError() == cudaSuccess ? TMS_OK : TMS_ERR_CUDA;
+}
+
+// workspace: [16-byte header][the re-laid-out table lutT]
+int launch_pq_smem(const PqArgs& a, void* workspace, bool f16) {
+    const DeviceInfo* di = device_info();
+    if (!di) return TMS_ERR_CUDA;
+    if (a.B == 0) return TMS_OK;
+    uint32_t* hdr = static_cast<uint32_t*>(workspace);
+    void* lutT = static_cast<uint8_t*>(workspace) + 16;
+    const int64_t total = (int64_t)a.Q * a.Nq * PQS_M * PQS_K;
+    if (f16) {
+        if (cudaMemsetAsync(hdr, 0, 16, a.stream) != cudaSuccess) return TMS_ERR_CUDA;
+        int64_t nb = (total + 1023) / 1024;
+        if (nb > 4 * di->num_sms) nb = 4 * di->num_sms;
+        pq_absmax_kernel<<<(unsigned)nb, 256, 0, a.stream>>>(a.lut, total, hdr);
+        pq_relayout_f16_kernel<<<(unsigned)((total + 255) / 256), 256, 0, a.stream>>>(a.lut, static_cast<__half*>(lutT),
+                                                                                     total, hdr);
+        count_launch(2);
+        if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+        return launch_pq_smem_t<true>(a, lutT, reinterpret_cast<const float*>(hdr + 1), di);
+    }
+    pq_relayout_kernel<<<(unsigned)((total + 255) / 256), 256, 0, a.stream>>>(a.lut, static_cast<float*>(lutT), total);
+    count_launch();
+    if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+    return launch_pq_smem_t<false>(a, lutT, nullptr, di);
 }
 
 }  // namespace tms

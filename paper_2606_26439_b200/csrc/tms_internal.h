@@ -64,9 +64,10 @@ struct PqArgs {
 int launch_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtype, const float* codebooks, int M,
                         int K, float* lut, cudaStream_t stream);
 int launch_pq_simt(const PqArgs& a);
-bool pq_smem_supports(const PqArgs& a);
+// f16: table entries stored as scaled fp16 (16 query rows per shared-memory slice, Nq % 16 == 0)
+bool pq_smem_supports(const PqArgs& a, bool f16);
 size_t pq_smem_workspace_bytes(int Q, int Nq);
-int launch_pq_smem(const PqArgs& a, void* workspace);
+int launch_pq_smem(const PqArgs& a, void* workspace, bool f16);
 
 // ---- top-k (csrc/topk.cu) ---------------------------------------------------------------------------------------
 size_t topk_workspace_bytes(int Q, int64_t B, int k);

@@ -15,8 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libtms.so")
 
 TMS_OK = 0
 TMS_DTYPE_F32, TMS_DTYPE_F16, TMS_DTYPE_BF16 = 0, 1, 2
-TMS_VARIANT_AUTO, TMS_VARIANT_SIMT, TMS_VARIANT_TCGEN05, TMS_VARIANT_PQ_SMEM = 0, 1, 2, 3
-VARIANTS = {"auto": 0, "simt": 1, "tcgen05": 2, "pq_smem": 3}
+TMS_VARIANT_AUTO, TMS_VARIANT_SIMT, TMS_VARIANT_TCGEN05, TMS_VARIANT_PQ_SMEM, TMS_VARIANT_PQ_SMEM_F16 = 0, 1, 2, 3, 4
+VARIANTS = {"auto": 0, "simt": 1, "tcgen05": 2, "pq_smem": 3, "pq_smem_f16": 4}
 
 _DTYPES = {torch.float32: TMS_DTYPE_F32, torch.float16: TMS_DTYPE_F16, torch.bfloat16: TMS_DTYPE_BF16}
 

@@ -47,7 +47,7 @@ def test_status_strings_and_version(lib):
 
 def test_workspace_size_functions(lib):
     assert lib.tms_maxsim_workspace_bytes(8, 32, 128, 500000, tms.TMS_DTYPE_BF16) == 0
-    assert lib.tms_pq_workspace_bytes(8, 32, 16, 256, 1000000) == 8 * 32 * 16 * 256 * 4
+    assert lib.tms_pq_workspace_bytes(8, 32, 16, 256, 1000000) == 8 * 32 * 16 * 256 * 4 + 16  # table + header
     assert lib.tms_pq_workspace_bytes(8, 32, 8, 256, 1000) == 0
     assert lib.tms_maxsim_host_workspace_min_bytes(8, 32, 128, tms.TMS_DTYPE_BF16, 180) > 2 * 180 * 256
 

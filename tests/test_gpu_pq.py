@@ -42,7 +42,7 @@ def test_lut_matches_eq8_in_fp64(q_dtype):
     assert np.abs(lut - ref).max() < 2e-6  # fp32 FMA chain of 8 terms, |terms| < 1
 
 
-@pytest.mark.parametrize("variant", ["simt", "pq_smem"])
+@pytest.mark.parametrize("variant", ["simt", "pq_smem", "pq_smem_f16"])
 def test_config4_shape_small(variant):
     off = synth.uniform_offsets(3000, 128)
     q, C, codes = pq_case(8, 32, 16, 256, 8, off, seed=3)
@@ -51,7 +51,7 @@ def test_config4_shape_small(variant):
     assert 28.0 < got.mean() < 31.0
 
 
-@pytest.mark.parametrize("variant", ["simt", "pq_smem"])
+@pytest.mark.parametrize("variant", ["simt", "pq_smem", "pq_smem_f16"])
 def test_ragged_documents(variant):
     lens = np.concatenate([[5, 128, 1, 0, 300, 16, 17, 15, 0, 0, 33, 1000],
                            synth.lognormal_lengths(2000, seed=2, median=40, lo=0, hi=200)])
@@ -77,6 +77,40 @@ def test_smem_and_general_kernels_agree_and_are_reproducible():
     _, b = run_pq(q, C, codes, off, "simt")
     assert np.array_equal(a, a2)
     assert np.abs(a - b).max() < 1e-4  # same fp32 terms, different summation order over m
+
+
+def test_f16_table_entries_stay_well_inside_the_16_bit_tolerance():
+    """TMS_VARIANT_PQ_SMEM_F16 rounds each stored table entry to fp16 (after a power-of-two block scale) and adds in
+    fp32: measured against the fp64 oracle and against the fp32-entry kernel on config 4's distribution."""
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(5000, seed=9))
+    q, C, codes = pq_case(8, 32, 16, 256, 8, off, seed=11)
+    ref = oracle.pq_maxsim(q, C, codes, off)
+    _, h = run_pq(q, C, codes, off, "pq_smem_f16")
+    _, h2 = run_pq(q, C, codes, off, "pq_smem_f16")
+    _, f = run_pq(q, C, codes, off, "pq_smem")
+    assert np.array_equal(h, h2)
+    assert np.abs(h - ref).max() <= 0.25 * 2e-3 * 32   # a quarter of the north_star tolerance
+    assert np.abs(h - f).max() <= 0.25 * 2e-3 * 32
+
+
+@pytest.mark.parametrize("scale", [1e-6, 1.0, 3e5])
+def test_f16_table_is_block_scaled(scale):
+    """The fp16 table is scaled by a power of two taken from max|lut|: codebooks of any magnitude neither overflow fp16
+    (3e5 * entries ~ 1e5 > 65504) nor fall into its subnormals (1e-6); the error stays relative to the scores."""
+    off = synth.offsets_from_lengths(synth.lognormal_lengths(1500, seed=21, lo=0))
+    q, C, codes = pq_case(4, 16, 16, 256, 8, off, seed=23)
+    C = (C * scale).contiguous()
+    ref = oracle.pq_maxsim(q, C, codes, off)
+    _, h = run_pq(q, C, codes, off, "pq_smem_f16")
+    assert_close(h / scale, ref / scale, 0.25 * 2e-3 * 16)
+
+
+def test_f16_table_needs_whole_16_row_slices():
+    off = synth.uniform_offsets(50, 20)
+    q, C, codes = pq_case(2, 24, 16, 256, 8, off, seed=25)   # Nq = 24: fine for the fp32 table (8-row slices) only
+    run_pq(q, C, codes, off, "pq_smem")
+    with pytest.raises(RuntimeError):
+        run_pq(q, C, codes, off, "pq_smem_f16")
 
 
 def test_p13_lossless_codes_reproduce_the_dense_path():
