@@ -157,9 +157,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         : "memory");
 }
 
-__device__ __forceinline__ uint4 ldg_codes(const uint8_t* p) {
+// A chunk's codes are read once per table slice: every pass but the last asks L2 to keep the lines (evict_last), the last
+// one marks them evict_first, so the chunk comes from HBM once even when 148 CTAs x 512 KB of live codes crowd L2.
+__device__ __forceinline__ uint4 ldg_codes(const uint8_t* p, uint64_t policy) {
     uint4 r;
-    asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p), "l"(policy));
     return r;
 }
 
@@ -211,6 +215,9 @@ pq_smem_kernel(const void* __restrict__ lutT, int Q, int Nq, const uint8_t* __re
     }
     uint32_t phase = 0;
     const float unscale = H16 ? *inv_scale : 1.f;
+    uint64_t pol_keep, pol_drop;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_drop));
     __syncthreads();
 
     for (int64_t chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
@@ -235,6 +242,7 @@ pq_smem_kernel(const void* __restrict__ lutT, int Q, int Nq, const uint8_t* __re
             mbar_wait(bar_a, phase);
             phase ^= 1;
 
+            const uint64_t pol = sl + 1 < nslices ? pol_keep : pol_drop;
             const int q = (sl * PQS_ROWS) / Nq;
             const bool first = (sl * PQS_ROWS) % Nq == 0;
             for (int dd = warp; dd < nd; dd += PQS_WARPS) {
@@ -243,14 +251,14 @@ pq_smem_kernel(const void* __restrict__ lutT, int Q, int Nq, const uint8_t* __re
                 const uint8_t* cp = codes + (t0 + slot) * PQS_M;
                 float part;
                 uint4 c = make_uint4(0, 0, 0, 0);
-                if (slot < n) c = ldg_codes(cp);
+                if (slot < n) c = ldg_codes(cp, pol);
                 if constexpr (H16) {
                     float r[8];
 #pragma unroll
                     for (int j = 0; j < 8; ++j) r[j] = -INFINITY;
                     for (int tb = 0; tb < n; tb += 16) {
                         uint4 cn = make_uint4(0, 0, 0, 0);
-                        if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M);  // prefetch next step
+                        if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M, pol);  // prefetch next step
                         float a[8];
 #pragma unroll
                         for (int j = 0; j < 8; ++j) a[j] = 0.f;
@@ -284,7 +292,7 @@ pq_smem_kernel(const void* __restrict__ lutT, int Q, int Nq, const uint8_t* __re
                 float r0 = -INFINITY, r1 = -INFINITY, r2 = -INFINITY, r3 = -INFINITY;
                 for (int tb = 0; tb < n; tb += 16) {
                     uint4 cn = make_uint4(0, 0, 0, 0);
-                    if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M);  // prefetch next step
+                    if (tb + 16 + slot < n) cn = ldg_codes(cp + (int64_t)(tb + 16) * PQS_M, pol);  // prefetch next step
                     float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
                     const uint32_t w[4] = {c.x, c.y, c.z, c.w};
 #pragma unroll

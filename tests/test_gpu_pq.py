@@ -155,8 +155,10 @@ def test_decode_variant_matches_the_oracle_and_the_lut_path(q_dtype, Q):
     assert_close(got, ref, 2e-3 * 32)
     fin = np.isfinite(ref)
     assert np.abs(got[fin] - ref[fin]).max() < 2e-4  # hi/lo split: far inside the tolerance
-    _, lut_scores = run_pq(q, C, codes, off)
+    _, lut_scores = run_pq(q, C, codes, off, "pq_smem")       # the LUT kernel over fp32 table entries
     assert np.abs(got[fin] - lut_scores[fin]).max() < 2e-4
+    _, auto_scores = run_pq(q, C, codes, off)                 # what tms_pq_maxsim runs by default: fp16 table entries
+    assert np.abs(got[fin] - auto_scores[fin]).max() <= 0.25 * 2e-3 * 32
 
 
 def test_decode_variant_exact_on_integer_codebooks():
