@@ -28,6 +28,8 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cstdlib>
+#include <cstring>
+#include <mutex>
 #include <cuda_runtime.h>
 
 #include "tms_internal.h"
@@ -269,24 +271,43 @@ __device__ __forceinline__ uint4 ldg_nc16(const void* p) {
 constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
 constexpr uint32_t DESC_LO = 1u << 16;
 
-// smallest b in [0, B] with offsets[b] >= target; whole warp, 32 probes per round
-__device__ int64_t warp_lower_bound(const int64_t* __restrict__ offsets, int64_t B, int64_t target, int lane) {
-    int64_t lo = 0, hi = B;  // the answer lies in [lo, hi]; offsets[B] = T >= target always holds
-    while (hi - lo > 32) {
-        const int64_t n = hi - lo;
-        const int64_t p = lo + (n * (lane + 1)) / 33;  // lo <= p < hi, increasing in lane
-        const bool ge = offsets[p] >= target;
-        const unsigned ball = __ballot_sync(0xffffffffu, ge);
-        const int f = ball ? __ffs(ball) - 1 : 32;
-        const int64_t p_f = __shfl_sync(0xffffffffu, p, f & 31);
-        const int64_t p_fm1 = __shfl_sync(0xffffffffu, p, (f - 1) & 31);
-        if (f < 32) hi = p_f;
-        if (f > 0) lo = p_fm1 + 1;
+// One 33-ary search state: the answer (smallest b in [0, B] with offsets[b] >= target) lies in [lo, hi]; val = offsets[hi].
+struct Search {
+    int64_t lo, hi, val, target;
+};
+// one round of 32 probes (n = hi - lo > 32): x is this lane's probe value at p = lo + n*(lane+1)/33
+__device__ __forceinline__ int64_t search_probe(const Search& s, int lane) { return s.lo + ((s.hi - s.lo) * (lane + 1)) / 33; }
+__device__ __forceinline__ void search_narrow(Search& s, int64_t p, int64_t x, int lane) {
+    const unsigned ball = __ballot_sync(0xffffffffu, x >= s.target);
+    const int f = ball ? __ffs(ball) - 1 : 32;
+    const int64_t p_f = __shfl_sync(0xffffffffu, p, f & 31), x_f = __shfl_sync(0xffffffffu, x, f & 31);
+    const int64_t p_fm1 = __shfl_sync(0xffffffffu, p, (f - 1) & 31);
+    if (f < 32) { s.hi = p_f; s.val = x_f; }
+    if (f > 0) s.lo = p_fm1 + 1;
+}
+// Both ends of a CTA's document range at once: the two searches run in lockstep so that their (dependent) global loads
+// overlap, and each returns offsets[answer] with the index, so no further load follows -- the prologue of a small batch
+// is a chain of ~3 load latencies instead of ~8.  offsets[B] = T is known without a load.
+__device__ void warp_lower_bound2(const int64_t* __restrict__ offsets, int64_t B, int64_t T, int64_t target_a,
+                                  int64_t target_b, int lane, int64_t& idx_a, int64_t& val_a, int64_t& idx_b,
+                                  int64_t& val_b) {
+    Search a{0, B, T, target_a}, b{0, B, T, target_b};
+    while (a.hi - a.lo > 32 || b.hi - b.lo > 32) {
+        const bool ra = a.hi - a.lo > 32, rb = b.hi - b.lo > 32;  // warp-uniform
+        const int64_t pa = ra ? search_probe(a, lane) : 0, pb = rb ? search_probe(b, lane) : 0;
+        const int64_t xa = ra ? offsets[pa] : 0, xb = rb ? offsets[pb] : 0;
+        if (ra) search_narrow(a, pa, xa, lane);
+        if (rb) search_narrow(b, pb, xb, lane);
     }
-    const int64_t p = lo + lane;
-    const bool ge = (p < hi) && (offsets[p] >= target);
-    const unsigned ball = __ballot_sync(0xffffffffu, ge);
-    return ball ? lo + (__ffs(ball) - 1) : hi;
+    const int64_t qa = a.lo + lane, qb = b.lo + lane;
+    const int64_t xa = qa < a.hi ? offsets[qa] : INT64_MAX, xb = qb < b.hi ? offsets[qb] : INT64_MAX;
+    const unsigned ba = __ballot_sync(0xffffffffu, qa < a.hi && xa >= a.target);
+    const unsigned bb = __ballot_sync(0xffffffffu, qb < b.hi && xb >= b.target);
+    const int64_t xa_f = __shfl_sync(0xffffffffu, xa, ba ? __ffs(ba) - 1 : 0), xb_f = __shfl_sync(0xffffffffu, xb, bb ? __ffs(bb) - 1 : 0);
+    idx_a = ba ? a.lo + (__ffs(ba) - 1) : a.hi;
+    val_a = ba ? xa_f : a.val;
+    idx_b = bb ? b.lo + (__ffs(bb) - 1) : b.hi;
+    val_b = bb ? xb_f : b.val;
 }
 
 struct SegInfo {
@@ -593,13 +614,15 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // work partition (a3): documents [b_lo, b_hi) whose first tokens lie in [c*T/G, (c+1)*T/G)
         const int64_t G = gridDim.x, c = blockIdx.x;
         const int64_t tgt_lo = (c * p.T) / G, tgt_hi = ((c + 1) * p.T) / G;
-        const int64_t b_lo = (c == 0) ? 0 : warp_lower_bound(p.offsets, p.B, tgt_lo, lane);
-        const int64_t b_hi = (c == G - 1) ? p.B : warp_lower_bound(p.offsets, p.B, tgt_hi, lane);
+        int64_t b_lo, b_hi, o_lo, o_hi;
+        warp_lower_bound2(p.offsets, p.B, p.T, tgt_lo, tgt_hi, lane, b_lo, o_lo, b_hi, o_hi);
+        if (c == 0) { b_lo = 0; o_lo = 0; }          // offsets[0] = 0
+        if (c == G - 1) { b_hi = p.B; o_hi = p.T; }  // offsets[B] = T
         if (lane == 0) {
             range[0] = b_lo;
             range[1] = b_hi;
-            range[2] = p.offsets[b_lo];
-            range[3] = p.offsets[b_hi];
+            range[2] = o_lo;
+            range[3] = o_hi;
         }
     } else if (warp == 1) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
@@ -1197,6 +1220,63 @@ bool make_map_2d(CUtensorMap* map, tms_dtype dtype, const void* base, uint64_t r
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Small-batch latency: encoding a tensor map and setting a kernel attribute cost microseconds of host time per call, as
+// much as a 1,000-document batch takes on the device.  Both depend only on (store address, shape, dtype) / (kernel,
+// device), so recent results are kept per process.  A tensor map holds no data, only the address and the geometry.
+struct MapKey {
+    const void* base;
+    uint64_t rows, cols;
+    uint32_t box_cols, box_rows;
+    int dtype, device;
+};
+struct MapEntry {
+    MapKey key;
+    CUtensorMap map;
+    bool valid;
+};
+std::mutex g_cache_mu;
+MapEntry g_maps[8];
+int g_map_next = 0;
+
+bool cached_map_2d(CUtensorMap* map, int device, tms_dtype dtype, const void* base, uint64_t rows, uint64_t cols,
+                   uint32_t box_cols, uint32_t box_rows) {
+    MapKey key;
+    memset(&key, 0, sizeof(key));  // padding bytes take part in the comparison
+    key.base = base; key.rows = rows; key.cols = cols; key.box_cols = box_cols; key.box_rows = box_rows;
+    key.dtype = (int)dtype; key.device = device;
+    std::lock_guard<std::mutex> lock(g_cache_mu);
+    for (const MapEntry& e : g_maps)
+        if (e.valid && memcmp(&e.key, &key, sizeof(key)) == 0) { *map = e.map; return true; }
+    if (!make_map_2d(map, dtype, base, rows, cols, box_cols, box_rows)) return false;
+    MapEntry& e = g_maps[g_map_next];
+    g_map_next = (g_map_next + 1) % 8;
+    e.key = key; e.map = *map; e.valid = true;
+    return true;
+}
+
+struct AttrEntry {
+    const void* kern;
+    int device;
+    uint32_t smem;
+};
+AttrEntry g_attrs[32];
+int g_nattrs = 0;
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize >= smem for this kernel on this device (set once per growth)
+bool ensure_smem_attr(const void* kern, int device, uint32_t smem) {
+    std::lock_guard<std::mutex> lock(g_cache_mu);
+    for (int i = 0; i < g_nattrs; ++i)
+        if (g_attrs[i].kern == kern && g_attrs[i].device == device) {
+            if (g_attrs[i].smem >= smem) return true;
+            if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+            g_attrs[i].smem = smem;
+            return true;
+        }
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+    if (g_nattrs < 32) g_attrs[g_nattrs++] = AttrEntry{kern, device, smem};
+    return true;
+}
+
 int next_pow2(int v) {
     int p = 1;
     while (p < v) p <<= 1;
@@ -1351,8 +1431,8 @@ int launch_dense_tc(const DenseArgs& a) {
     if (di->cc_major != 10 || !plan(a, pl) || pl.smem_bytes > (uint32_t)di->max_smem_optin) return TMS_ERR_UNSUPPORTED;
 
     CUtensorMap map_docs = {};  // unused by the PQ decode variant
-    if (!pl.pqd &&
-        !make_map_2d(&map_docs, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d, (uint32_t)pl.p.kb_elems, BN))
+    if (!pl.pqd && !cached_map_2d(&map_docs, di->device, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d,
+                                  (uint32_t)pl.p.kb_elems, BN))
         return TMS_ERR_CUDA;
 
     void (*kern)(const CUtensorMap, const Params) = nullptr;
@@ -1365,8 +1445,7 @@ int launch_dense_tc(const DenseArgs& a) {
         if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 2> : dense_tc_kernel<1, 2, false, false, 2>;
         else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 2> : dense_tc_kernel<2, 2, false, false, 2>;
     }
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess)
-        return TMS_ERR_CUDA;
+    if (!ensure_smem_attr(reinterpret_cast<const void*>(kern), di->device, pl.smem_bytes)) return TMS_ERR_CUDA;
     // no more CTAs than 128-token tiles; one CTA per SM
     int64_t grid = (a.T + BN - 1) / BN;
     if (grid > di->num_sms) grid = di->num_sms;
