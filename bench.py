@@ -45,6 +45,10 @@ WORKLOADS = {
     "c4-d256": dict(kind="dense", Q=4, Nq=32, d=256, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "c4-d512": dict(kind="dense", Q=4, Nq=32, d=512, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "c4-d768": dict(kind="dense", Q=4, Nq=32, d=768, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    # the dimension sweep at Q=8: two query blocks do not fit tensor memory next to the accumulators for d > 256, so the
+    # kernel runs as CTA pairs that share every document tile by TMA multicast (the store is still read once)
+    "c4-d512-q8": dict(kind="dense", Q=8, Nq=32, d=512, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
+    "c4-d768-q8": dict(kind="dense", Q=8, Nq=32, d=768, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     # NEXT-1: the paper's query-length and document-length sweeps (Tables 10, 11), Q=1 as in the paper
     "n1-nq8": dict(kind="dense", Q=1, Nq=8, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
     "n1-nq16": dict(kind="dense", Q=1, Nq=16, d=128, dtype="bf16", B=100_000, Nd=128, lengths="uniform"),
@@ -459,7 +463,7 @@ def roofline_of(wl, step_ms, total_ms, clocks, peaks):
 
 
 SECONDARY = ["c2-q4", "c2-q1", "c2-fp16", "c2-fp32", "c3-100k", "c3-250k", "c3-500k", "c4-d64", "c4-d256", "c4-d512",
-             "c4-d768", "c5", "c5-f32", "c5-decode", "c5-decode-fp16"]
+             "c4-d768", "c4-d512-q8", "c4-d768-q8", "c5", "c5-f32", "c5-decode", "c5-decode-fp16"]
 
 
 def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):

@@ -79,11 +79,13 @@ typedef enum {
  *               live in the workspace and are added by a second kernel.  A workspace that is missing or too
  *               small for such a shape is TMS_ERR_WORKSPACE, a mis-aligned one TMS_ERR_ALIGNMENT -- the call
  *               never switches to a slower kernel because of its scratch.
- * Every document embedding is read from HBM once per group of query rows that fits tensor memory next to
- * its accumulators: 256 rows (Q*Nq, Nq rounded up to a power of two) for d*sizeof(dtype) <= 512 bytes, 128 rows
- * beyond that (16-bit d in (256, 768], where the query block alone takes 192..384 of the 512 columns); a call with
- * more rows runs ceil(rows / group) launches, each streaming the store once -- the ceil(Nq/BQ) factor of Thm 1
- * (P:L228).  No similarity matrix is written to memory (Eq. 7).
+ * Every document embedding is read from HBM once per group of up to 256 query rows (Q*Nq, Nq rounded up to a power of
+ * two): for d*sizeof(dtype) <= 512 bytes both 128-row blocks sit in one SM's tensor memory next to their accumulators;
+ * for 16-bit d in (256, 768] only one block fits, and 256 rows run as clusters of two CTAs -- one block each -- that
+ * share every document tile by TMA multicast, so the store still crosses the HBM interface once.  fp32 inputs with
+ * d > 128 keep one block per launch (128 rows).  A call with more rows runs ceil(rows / group) launches, each
+ * streaming the store once -- the ceil(Nq/BQ) factor of Thm 1.  No similarity matrix is written to memory
+ * (Eq. 7).
  * d > 128 accumulates partial dot products over dimension chunks before the max is taken.
  */
 int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,

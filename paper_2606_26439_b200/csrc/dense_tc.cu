@@ -152,6 +152,25 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "l"(map), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
         : "memory");
 }
+// The same copy delivered to the same shared-memory offset of every CTA of the cluster named in cta_mask; each
+// destination CTA's mbarrier (same offset) receives the bytes that landed in it.
+__device__ __forceinline__ void tma_load_2d_multicast(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1,
+                                                      uint16_t cta_mask, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint"
+        " [%0], [%1, {%4, %5}], [%2], %3, %6;" ::"r"(dst),
+        "l"(map), "r"(bar), "h"(cta_mask), "r"(c0), "r"(c1), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// every thread of every CTA of the cluster
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 // 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (size and addresses multiples of 16)
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -173,6 +192,12 @@ __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence:
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// the same arrive on the mbarrier at this shared-memory offset in every CTA of cta_mask (a CTA pair shares stages)
+__device__ __forceinline__ void tc_commit_multicast(uint32_t bar, uint16_t cta_mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"(cta_mask)
+                 : "memory");
 }
 // D[tmem] (+)= A[tmem] . B[smem]^T, kind::f16 (fp16/bf16 in, fp32 accumulate)
 __device__ __forceinline__ void tc_mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
@@ -560,9 +585,17 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
 // because of its HBM round trip; on-chip it costs 16 bytes of HBM per token and no lookup per query row).
 // NSET: epilogue warp sets.  2 (16-bit inputs only): two warps per 32 TMEM lanes, one per half of a tile's columns --
 // pays when documents are short (many boundaries per tile: the segmented reduction is the binding step); 1 otherwise.
-template <int MB, int KBS, bool F32, bool PQD, int NSET>
+// PAIR (16-bit inputs, MB = 1): "read once" for 256 query rows when d is too large for two resident query blocks
+// (d*sizeof > 512 bytes).  The kernel runs as clusters of two CTAs that walk the SAME token range; CTA r keeps query
+// block r in its tensor memory, loads HALF of every document tile (64 tokens) and multicasts it into both CTAs'
+// shared memory, so the pair reads each embedding from L2/HBM once and each SM contracts it against its own 128 rows.
+// A stage is shared state: it is refilled only when BOTH CTAs' tensor pipes have read it (the `empty` barriers count two
+// arrivals, each CTA's tcgen05.commit is multicast to both).  Everything else -- MMA issue, segmenter, epilogue, max->sum
+// -- is per CTA and unchanged (Thm 1's ceil(Nq/BQ) factor stays 1).
+template <int MB, int KBS, bool F32, bool PQD, int NSET, bool PAIR = false>
 __global__ void __launch_bounds__(128 + NSET * 128 * MB + (F32 ? 128 : 0), 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
+    static_assert(!PAIR || (MB == 1 && !F32 && !PQD), "CTA pairs: one query block per CTA, 16-bit inputs");
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -595,11 +628,12 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     int64_t* range = reinterpret_cast<int64_t*>(carry + 17);  // b_lo, b_hi, t_lo, t_hi
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = PAIR ? cluster_ctarank() : 0u;  // which query block (and which half of every tile) is this CTA's
 
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0) {
         if (lane == 0) {
-            for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), F32 ? 4 : 1); mbar_init(smem_u32(empty + s), 1); }
+            for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), F32 ? 4 : 1); mbar_init(smem_u32(empty + s), PAIR ? 2 : 1); }
             for (int s = 0; s < 8; ++s) mbar_init(smem_u32(tfull + s), 1);
             for (int s = 0; s < MAX_ACC; ++s) mbar_init(smem_u32(tempty + s), 4 * NSET);
             for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
@@ -612,7 +646,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             if (!PQD) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_docs) : "memory");
         }
         // work partition (a3): documents [b_lo, b_hi) whose first tokens lie in [c*T/G, (c+1)*T/G)
-        const int64_t G = gridDim.x, c = blockIdx.x;
+        const int64_t G = PAIR ? gridDim.x >> 1 : gridDim.x, c = PAIR ? blockIdx.x >> 1 : blockIdx.x;  // a pair shares its range
         const int64_t tgt_lo = (c * p.T) / G, tgt_hi = ((c + 1) * p.T) / G;
         int64_t b_lo, b_hi, o_lo, o_hi;
         warp_lower_bound2(p.offsets, p.B, p.T, tgt_lo, tgt_hi, lane, b_lo, o_lo, b_hi, o_hi);
@@ -631,7 +665,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
-    __syncthreads();
+    if constexpr (PAIR) cluster_sync_all();  // the peer's barriers are initialised before anything is sent to them
+    else __syncthreads();
     tc_fence_after();
 
     const uint32_t tmem_base = *tmem_slot;
@@ -681,11 +716,17 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     } else
 #endif
                     if (elect_one()) {
-                        mbar_expect_tx(smem_u32(full + s), stage_bytes);
+                        mbar_expect_tx(smem_u32(full + s), stage_bytes);  // both halves land here: mine and the peer's
 #pragma unroll
-                        for (int k = 0; k < KBS; ++k)
-                            tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
-                                        smem_u32(full + s), (ch * KBS + k) * p.kb_elems, tok, pol_docs);
+                        for (int k = 0; k < KBS; ++k) {
+                            if constexpr (PAIR)  // token rows [64*rank, +64) of the tile, into both CTAs
+                                tma_load_2d_multicast(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES) + rank * (KB_TILE_BYTES / 2),
+                                                      &map_docs, smem_u32(full + s), (ch * KBS + k) * p.kb_elems,
+                                                      tok + (int)rank * (BN / 2), (uint16_t)3, pol_docs);
+                            else
+                                tma_load_2d(smem_u32(st_ptr + (size_t)s * stage_bytes + k * KB_TILE_BYTES), &map_docs,
+                                            smem_u32(full + s), (ch * KBS + k) * p.kb_elems, tok, pol_docs);
+                        }
                     }
                 }
                 __syncwarp();
@@ -718,7 +759,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // TMEM columns of one query block's rows (F32: hi halves of all units, then lo halves)
         const uint32_t a_lo_off = (uint32_t)p.NKB * KB_WORDS;
         const uint32_t a_mb_step = F32 ? 2 * a_lo_off : a_lo_off;
-        const bool epi_frees_stage = !F32 && nchunks == 1;
+        const bool epi_frees_stage = !F32 && !PAIR && nchunks == 1;
         const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), tempty0 = smem_u32(tempty), tfull0 = smem_u32(tfull);
         const uint32_t my_turn = smem_u32(turn + w), other_turn = smem_u32(turn + (w ^ 1));
         // ring positions of this warp's first tile (tile w): operand stage w*nchunks, accumulator jobs w*MB + mb
@@ -792,7 +833,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         // the epilogue that the stage has been read (it hands the stage back to the producer): one
                         // tcgen05.commit fewer per tile.
                         if (last_chunk) tc_commit(tfull0 + (tq * MB + mb) * 8);
-                        if (mb == MB - 1 && !epi_frees_stage) tc_commit(empty0 + s * 8);
+                        if (mb == MB - 1 && !epi_frees_stage) {
+                            if constexpr (PAIR) tc_commit_multicast(empty0 + s * 8, (uint16_t)3);  // the stage is the pair's
+                            else tc_commit(empty0 + s * 8);
+                        }
                         if (last_chunk && mb == MB - 1) mbar_arrive(other_turn);  // the other issuer may start its tile
                     }
                     __syncwarp();
@@ -817,6 +861,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         // loaded one window ahead, so no tile waits on a global load.  A document's start is its predecessor's end.
         const uint32_t lt_mask = (1u << lane) - 1u;
         const float ninf = -INFINITY;
+        // the queries whose scores this CTA writes: all of the launch's, or (CTA pairs) those of its own query block
+        const int q_first = PAIR ? (int)rank * (128 / p.Nq_pad) : 0;
+        const int q_end = PAIR ? (p.Q < q_first + 128 / p.Nq_pad ? p.Q : q_first + 128 / p.Nq_pad) : p.Q;
         const int64_t never = INT64_MAX;
         auto load_ends = [&](int64_t base) -> int64_t {
             const int64_t idx = base + lane;
@@ -849,7 +896,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     w0 = (col >> 5) == 0 ? bit : 0; w1 = (col >> 5) == 1 ? bit : 0;
                     w2 = (col >> 5) == 2 ? bit : 0; w3 = (col >> 5) == 3 ? bit : 0;
                 } else if (in_tile) {
-                    for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;  // empty document (A2)
+                    for (int q = q_first; q < q_end; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;  // empty document (A2)
                 }
                 if (nb) {
                     m0 |= __reduce_or_sync(0xffffffffu, w0); m1 |= __reduce_or_sync(0xffffffffu, w1);
@@ -871,7 +918,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         }
         // documents after the last token of the range can only be empty
         for (int64_t idx = wb + consumed + lane; idx < b_hi; idx += 32)
-            for (int q = 0; q < p.Q; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
+            for (int q = q_first; q < q_end; ++q) p.scores[(int64_t)q * p.B + idx] = ninf;
     } else if (F32 && warp >= 4 + NSET * n_epi_warps) {
         // ===== fp32 splitter (F32 only): raw fp32 stage -> bf16 hi block + bf16 lo block of an operand stage =====
         // Thread r owns token row r of the tile.  Both layouts are the 128-byte swizzle (16-byte piece index XOR
@@ -969,7 +1016,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         int set = (warp - 4) / n_epi_warps;                  // which half of every tile's columns is this warp's (NSET == 2)
         if (NSET == 2) asm volatile("" : "+r"(set));           // opaque: otherwise re-derived from %tid.x (S2R) at every use
         const int ew = (warp - 4) % n_epi_warps, mb = ew >> 2, quad = warp & 3;
-        const int row = mb * 128 + quad * 32 + lane;   // this thread's query row = TMEM lane quad*32+lane of block mb
+        const int row = ((int)rank + mb) * 128 + quad * 32 + lane;   // this thread's query row = TMEM lane quad*32+lane of block mb
         const int q = row / p.Nq_pad, i = row - q * p.Nq_pad;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(quad * 32) << 16);
 
@@ -1037,7 +1084,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         }
 
         // max -> sum constants of this warp: its 32 rows hold 32/Nq_pad queries, the first one being q0
-        const int q0 = (mb * 128 + quad * 32) / p.Nq_pad;
+        const int q0 = (((int)rank + mb) * 128 + quad * 32) / p.Nq_pad;
         const int nsub = 32 / p.Nq_pad;
         const int nvalid = p.Q - q0 < 0 ? 0 : (p.Q - q0 < nsub ? p.Q - q0 : nsub);
         const uint32_t cfg = pack_cfg(p.Nq, p.Nq_pad, nvalid);
@@ -1046,7 +1093,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const bool skip_math = PROBE(p, 1);
         const int64_t B = p.B;
         const uint32_t ring = smem_u32(docring);
-        const bool frees_stage = !F32 && nchunks == 1 && set == 0 && ew == 4 * (MB - 1);  // see the MMA warps
+        const bool frees_stage = !F32 && !PAIR && nchunks == 1 && set == 0 && ew == 4 * (MB - 1);  // see the MMA warps
 
         // Two sets (16-bit inputs): set 0 reduces columns 0..63 of every tile, set 1 columns 64..127.  A tcgen05.ld
         // blocks the issuing warp until its data are in registers (measured: two loads "in flight" from one warp take
@@ -1168,7 +1215,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
 
     // ---- teardown --------------------------------------------------------------------------------------------
     tc_fence_before();
-    __syncthreads();
+    if constexpr (PAIR) cluster_sync_all();  // no CTA leaves while its peer can still signal its barriers
+    else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)TMEM_COLS)
@@ -1299,6 +1347,7 @@ struct Plan {
     int nparts;         // equal parts a query is scored in (1 unless Nq > 32)
     int Qg;             // queries per launch
     int nset;           // epilogue warp sets
+    bool pair;          // clusters of two CTAs, one query block each, document tiles multicast to both
     uint32_t smem_bytes;
 };
 
@@ -1334,6 +1383,9 @@ bool plan(const DenseArgs& a, Plan& pl) {
     if (MB * a_cols_per_block + MB * BN > TMEM_COLS) MB = 1;
     if (MB * a_cols_per_block + MB * BN > TMEM_COLS) return false;  // d too large for a resident query block
     const int per_block = 128 / nqp;  // queries per 128-row block
+    // two query blocks wanted but only one fits tensor memory (16-bit d in (256, 768]): a CTA pair holds one block each
+    // and shares the document tiles by multicast, so the store is still read once per 256 rows
+    const bool pair = !f32 && MB == 1 && a.Q * nparts > per_block;
     if (a.Q * nparts <= per_block) MB = 1;
     Params& p = pl.p;
     p.offsets = a.offsets;
@@ -1363,7 +1415,8 @@ bool plan(const DenseArgs& a, Plan& pl) {
     // instruction descriptor: fp32 accumulate, A/B format, both K-major, N = 128, M = 128
     p.idesc = (1u << 4) | (fmt << 7) | (fmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     pl.MB = MB;
-    pl.Qg = MB * per_block;
+    pl.pair = pair;
+    pl.Qg = (pair ? 2 : MB) * per_block;
     pl.nparts = nparts;
     pl.f32 = f32;
     pl.pqd = pqd;
@@ -1432,13 +1485,16 @@ int launch_dense_tc(const DenseArgs& a) {
 
     CUtensorMap map_docs = {};  // unused by the PQ decode variant
     if (!pl.pqd && !cached_map_2d(&map_docs, di->device, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d,
-                                  (uint32_t)pl.p.kb_elems, BN))
+                                  (uint32_t)pl.p.kb_elems, pl.pair ? BN / 2 : BN))  // a pair's CTAs load half a tile each
         return TMS_ERR_CUDA;
 
     void (*kern)(const CUtensorMap, const Params) = nullptr;
     if (pl.pqd) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, true, 1> : dense_tc_kernel<2, 2, true, true, 1>;
     else if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, false, 1> : dense_tc_kernel<2, 2, true, false, 1>;
-    else if (pl.nset == 1) {
+    else if (pl.pair) {
+        if (pl.nset == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 1, true> : dense_tc_kernel<1, 2, false, false, 1, true>;
+        else kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 2, true> : dense_tc_kernel<1, 2, false, false, 2, true>;
+    } else if (pl.nset == 1) {
         if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 1> : dense_tc_kernel<1, 2, false, false, 1>;
         else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 1> : dense_tc_kernel<2, 2, false, false, 1>;
     } else {
@@ -1449,6 +1505,11 @@ int launch_dense_tc(const DenseArgs& a) {
     // no more CTAs than 128-token tiles; one CTA per SM
     int64_t grid = (a.T + BN - 1) / BN;
     if (grid > di->num_sms) grid = di->num_sms;
+    if (pl.pair) {  // one range per pair of CTAs (the two SMs of a TPC)
+        int64_t pairs = (a.T + BN - 1) / BN;
+        if (pairs > di->num_sms / 2) pairs = di->num_sms / 2;
+        grid = 2 * pairs;
+    }
 #ifdef TMS_PROBES
     if (const char* e = getenv("TMS_GRID")) { const int g = atoi(e); if (g > 0 && g < grid) grid = g; }
     if (const char* e = getenv("TMS_NS")) { const int n = atoi(e); if (n > 0 && n < pl.p.NS) pl.p.NS = n; }
@@ -1461,9 +1522,21 @@ int launch_dense_tc(const DenseArgs& a) {
         p.Q = Qeff - q0 < pl.Qg ? Qeff - q0 : pl.Qg;
         p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * p.Nq * p.row_bytes;
         p.scores = dst + (int64_t)q0 * a.B;
-        kern<<<(unsigned)grid, 128 + pl.nset * 128 * pl.MB + (pl.f32 ? 128 : 0), pl.smem_bytes, a.stream>>>(map_docs, p);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid);
+        cfg.blockDim = dim3(128 + pl.nset * 128 * pl.MB + (pl.f32 ? 128 : 0));
+        cfg.dynamicSmemBytes = pl.smem_bytes;
+        cfg.stream = a.stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = pl.pair ? 2 : 1;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        const cudaError_t err = cudaLaunchKernelEx(&cfg, kern, map_docs, p);
         count_launch();
-        if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
+        if (err != cudaSuccess || cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
     }
     if (pl.nparts > 1) {
         const int64_t n = (int64_t)a.Q * a.B;

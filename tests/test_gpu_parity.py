@@ -145,6 +145,23 @@ def test_dimension_sweep(d, variant):
     assert_close(run_dense(q, D, off, variant), oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
 
 
+@pytest.mark.parametrize("d", [320, 384, 512, 768])
+@pytest.mark.parametrize("Q", [5, 8, 11])
+def test_two_query_blocks_at_large_d_run_as_cta_pairs(d, Q):
+    """d*sizeof > 512 bytes leaves tensor memory room for ONE 128-row query block per SM; 256 rows then run as clusters
+    of two CTAs that share every document tile by TMA multicast.  Same arithmetic per row as the
+    single-CTA kernel, so scoring the queries four at a time (one block, no pairs) must give identical bits."""
+    lens = np.concatenate([RAGGED, np.full(200, 128), synth.lognormal_lengths(700, seed=d + Q)])
+    off = synth.offsets_from_lengths(lens)
+    q, D = unit_case(Q, 32, d, torch.bfloat16, off, seed=d + 3 * Q)
+    got = run_dense(q, D, off, "tcgen05")
+    assert_close(got, oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
+    parts = [run_dense(q[i:i + 4], D, off, "tcgen05") for i in range(0, Q, 4)]
+    assert np.array_equal(got, np.concatenate(parts, axis=0))
+    again = run_dense(q, D, off, "tcgen05")
+    assert np.array_equal(got, again)
+
+
 def test_p11_zero_padded_dimensions_tie_the_tiled_variant_to_d128():
     off = synth.offsets_from_lengths(synth.lognormal_lengths(800, seed=3))
     q, D = unit_case(4, 32, 128, torch.bfloat16, off, seed=21)
