@@ -600,9 +600,12 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     // layout: [operand stages: NS * KBS*16 KB] [F32: raw stages: NR * 32 KB] [SegInfo x NSEG] [park buffers] [barriers]
-    constexpr uint32_t stage_bytes = (uint32_t)KBS * KB_TILE_BYTES;
+    // PQD with fp16 operands has no lo parts: its stages hold one 16 KB block and its codebook one 64 KB plane, which
+    // leaves room for eight operand stages instead of two (the decode then runs ahead of the tensor pipe).
+    const bool pq_half = PQD && p.half_mode != 0;
+    const uint32_t stage_bytes = pq_half ? (uint32_t)KB_TILE_BYTES : (uint32_t)KBS * KB_TILE_BYTES;
     constexpr uint32_t raw_bytes = PQD ? BN * 16u : 2u * KB_TILE_BYTES;  // PQD: 16 code bytes per token
-    constexpr uint32_t cb_bytes = PQD ? 16u * 256u * 8u * 4u : 0u;        // PQD: the codebook [16][256][8], as two bf16 planes
+    const uint32_t cb_bytes = PQD ? (pq_half ? 16u * 256u * 8u * 2u : 16u * 256u * 8u * 4u) : 0u;  // PQD: the codebook [16][256][8], as two bf16 planes (or one fp16 plane)
     constexpr int n_epi_warps = 4 * MB;            // epilogue warps of one set (one set reduces a tile)
     static_assert(NSET == 1 || (NSET == 2 && !F32), "two epilogue sets exist for 16-bit inputs only");
     uint8_t* st_ptr = smem;
@@ -950,7 +953,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                     encode_pair(__uint_as_float(y1.x), __uint_as_float(y1.y), hi.z, lo.z, half_mode);
                     encode_pair(__uint_as_float(y1.z), __uint_as_float(y1.w), hi.w, lo.w, half_mode);
                     *reinterpret_cast<uint4*>(cb_ptr + e * 16) = hi;
-                    *reinterpret_cast<uint4*>(cb_ptr + cb_bytes / 2 + e * 16) = lo;
+                    if (!half_mode) *reinterpret_cast<uint4*>(cb_ptr + cb_bytes / 2 + e * 16) = lo;
                 }
                 asm volatile("bar.sync 1, 128;" ::: "memory");  // the four splitter warps
             }
@@ -958,7 +961,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 mbar_wait(smem_u32(rfull + rs), rph);
                 const uint4 cw = *reinterpret_cast<const uint4*>(rw_ptr + (size_t)rs * raw_bytes + r * 16);
                 const uint32_t cword[4] = {cw.x, cw.y, cw.z, cw.w};
-                for (int ch = 0; ch < nchunks; ++ch) {
+#pragma unroll
+                for (int ch = 0; ch < 2; ++ch) {  // d = 128: two 64-dimension units per tile (compile-time: cword stays in registers)
                     mbar_wait(smem_u32(empty + s), ph ^ 1);
                     uint8_t* op = st_ptr + (size_t)s * stage_bytes + r * KB_BYTES;
 #pragma unroll
@@ -1431,13 +1435,15 @@ bool plan(const DenseArgs& a, Plan& pl) {
     const uint32_t stage_bytes = (uint32_t)pl.KBS * KB_TILE_BYTES;
     int ns = (int)((SMEM_LIMIT - fixed) / stage_bytes);
     p.NR = 0;
-    if (pqd) {  // 128 KB codebook + four 2 KB code stages, the rest for 32 KB operand stages
-        const uint32_t cb = 16u * 256u * 8u * 4u, raw = MAX_RAW * BN * 16u;
-        if (fixed + cb + raw + stage_bytes > SMEM_LIMIT) return false;
+    if (pqd) {  // 128 KB codebook + four 2 KB code stages, the rest for 32 KB operand stages (hi + lo block); with fp16
+                // operands there are no lo parts: 64 KB codebook, 16 KB stages
+        const uint32_t cb = p.half_mode ? 16u * 256u * 8u * 2u : 16u * 256u * 8u * 4u, raw = MAX_RAW * BN * 16u;
+        const uint32_t sb = p.half_mode ? (uint32_t)KB_TILE_BYTES : stage_bytes;
+        if (fixed + cb + raw + sb > SMEM_LIMIT) return false;
         p.NR = MAX_RAW;
-        ns = (int)((SMEM_LIMIT - fixed - cb - raw) / stage_bytes);
+        ns = (int)((SMEM_LIMIT - fixed - cb - raw) / sb);
         p.NS = ns > MAX_STAGES ? MAX_STAGES : ns;
-        pl.smem_bytes = (uint32_t)p.NS * stage_bytes + raw + cb + fixed;
+        pl.smem_bytes = (uint32_t)p.NS * sb + raw + cb + fixed;
         return p.NS >= 1;
     }
     if (f32) {  // 32 KB raw stages and 32 KB operand stages share the budget
