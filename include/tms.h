@@ -87,6 +87,9 @@ typedef enum {
  * streaming the store once -- the ceil(Nq/BQ) factor of Thm 1.  No similarity matrix is written to memory
  * (Eq. 7).
  * d > 128 accumulates partial dot products over dimension chunks before the max is taken.
+ * Stores of 2^31 - 128 tokens or more (TMA tile coordinates are 32-bit) are scored in segments of 2^30 tokens, one
+ * launch per segment; a single document must then be shorter than 2^30 tokens.  The same holds for
+ * tms_pq_maxsim_decode.
  */
 int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
                int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace, size_t workspace_bytes,
@@ -102,7 +105,7 @@ size_t tms_maxsim_workspace_bytes(int Q, int Nq, int d, int64_t B, tms_dtype dty
 
 /* Which kernel tms_maxsim (TMS_VARIANT_AUTO) runs for this shape on an sm_100 device, given an adequate workspace:
  * TMS_VARIANT_TCGEN05 or TMS_VARIANT_SIMT (the general CUDA-core kernel, far below the HBM roofline: d*sizeof(dtype)
- * beyond tensor-memory residency, fp32 with d % 64 != 0, total_tokens >= 2^31 - 128).  TMS_VARIANT_AUTO when nothing
+ * beyond tensor-memory residency, fp32 with d % 64 != 0).  TMS_VARIANT_AUTO when nothing
  * is scored (B == 0 or total_tokens == 0).  A pure function of its arguments: no device is touched. */
 int tms_maxsim_variant_used(int Q, int Nq, int d, int64_t B, int64_t total_tokens, tms_dtype dtype);
 

@@ -56,6 +56,10 @@ struct Params {
     const int64_t* offsets;
     float* scores;         // this launch's first score row
     int64_t B, T;
+    // Stores of 2^31 tokens or more (TMA coordinates are 32-bit) are scored in token segments, one launch each: this
+    // launch takes the documents whose FIRST token lies in [tok0, tok0 + Tseg); its tensor map starts at token tok0.
+    int64_t tok0, Tseg;
+    int seg_first, seg_last;  // the first segment owns leading empty documents, the last one trailing ones
     int Q, Nq, Nq_pad;     // queries in this launch
     int row_bytes;         // d * sizeof(element)
     int NKB;               // dimension blocks per row = row_bytes / 128
@@ -650,11 +654,11 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         }
         // work partition (a3): documents [b_lo, b_hi) whose first tokens lie in [c*T/G, (c+1)*T/G)
         const int64_t G = PAIR ? gridDim.x >> 1 : gridDim.x, c = PAIR ? blockIdx.x >> 1 : blockIdx.x;  // a pair shares its range
-        const int64_t tgt_lo = (c * p.T) / G, tgt_hi = ((c + 1) * p.T) / G;
+        const int64_t tgt_lo = p.tok0 + (c * p.Tseg) / G, tgt_hi = p.tok0 + ((c + 1) * p.Tseg) / G;
         int64_t b_lo, b_hi, o_lo, o_hi;
         warp_lower_bound2(p.offsets, p.B, p.T, tgt_lo, tgt_hi, lane, b_lo, o_lo, b_hi, o_hi);
-        if (c == 0) { b_lo = 0; o_lo = 0; }          // offsets[0] = 0
-        if (c == G - 1) { b_hi = p.B; o_hi = p.T; }  // offsets[B] = T
+        if (c == 0 && p.seg_first) { b_lo = 0; o_lo = 0; }          // offsets[0] = 0
+        if (c == G - 1 && p.seg_last) { b_hi = p.B; o_hi = p.T; }  // offsets[B] = T
         if (lane == 0) {
             range[0] = b_lo;
             range[1] = b_hi;
@@ -696,7 +700,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             if (++s == nring) { s = 0; ph ^= 1; }
         }
         for (int64_t t = 0; !PQD && t < ntiles; ++t) {
-            const int tok = (int)(t_lo + t * BN);
+            const int tok = (int)(t_lo - p.tok0 + t * BN);  // row of this launch's tensor map
             for (int ch = 0; ch < nchunks; ++ch) {
                 if constexpr (F32) {
                     mbar_wait(smem_u32(rempty + s), ph ^ 1);
@@ -1363,7 +1367,7 @@ uint32_t fixed_smem(int MB, int nset) {
 
 // Shape -> kernel parameters; false when the tcgen05 path does not cover it.
 bool plan(const DenseArgs& a, Plan& pl) {
-    if (a.B <= 0 || a.T <= 0 || a.T >= (1ll << 31) - BN) return false;
+    if (a.B <= 0 || a.T <= 0) return false;
     const bool pqd = a.codes != nullptr;  // decode-and-contract PQ: fp32-split machinery, 16-bit or fp32 queries
     if (pqd && (a.d != 128 || !a.codebooks)) return false;
     const bool f32 = pqd || a.dtype == TMS_DTYPE_F32;
@@ -1395,6 +1399,9 @@ bool plan(const DenseArgs& a, Plan& pl) {
     p.offsets = a.offsets;
     p.B = a.B;
     p.T = a.T;
+    p.tok0 = 0;
+    p.Tseg = a.T;
+    p.seg_first = p.seg_last = 1;
     p.Nq = Nq_part;
     p.Nq_pad = nqp;
     p.row_bytes = row_bytes;
@@ -1489,11 +1496,6 @@ int launch_dense_tc(const DenseArgs& a) {
     Plan pl;
     if (di->cc_major != 10 || !plan(a, pl) || pl.smem_bytes > (uint32_t)di->max_smem_optin) return TMS_ERR_UNSUPPORTED;
 
-    CUtensorMap map_docs = {};  // unused by the PQ decode variant
-    if (!pl.pqd && !cached_map_2d(&map_docs, di->device, a.dtype, a.docs, (uint64_t)a.T, (uint64_t)a.d,
-                                  (uint32_t)pl.p.kb_elems, pl.pair ? BN / 2 : BN))  // a pair's CTAs load half a tile each
-        return TMS_ERR_CUDA;
-
     void (*kern)(const CUtensorMap, const Params) = nullptr;
     if (pl.pqd) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, true, 1> : dense_tc_kernel<2, 2, true, true, 1>;
     else if (pl.f32) kern = pl.MB == 1 ? dense_tc_kernel<1, 2, true, false, 1> : dense_tc_kernel<2, 2, true, false, 1>;
@@ -1508,23 +1510,44 @@ int launch_dense_tc(const DenseArgs& a) {
         else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 2> : dense_tc_kernel<2, 2, false, false, 2>;
     }
     if (!ensure_smem_attr(reinterpret_cast<const void*>(kern), di->device, pl.smem_bytes)) return TMS_ERR_CUDA;
-    // no more CTAs than 128-token tiles; one CTA per SM
-    int64_t grid = (a.T + BN - 1) / BN;
-    if (grid > di->num_sms) grid = di->num_sms;
-    if (pl.pair) {  // one range per pair of CTAs (the two SMs of a TPC)
-        int64_t pairs = (a.T + BN - 1) / BN;
-        if (pairs > di->num_sms / 2) pairs = di->num_sms / 2;
-        grid = 2 * pairs;
-    }
-#ifdef TMS_PROBES
-    if (const char* e = getenv("TMS_GRID")) { const int g = atoi(e); if (g > 0 && g < grid) grid = g; }
-    if (const char* e = getenv("TMS_NS")) { const int n = atoi(e); if (n > 0 && n < pl.p.NS) pl.p.NS = n; }
-#endif
+    // TMA tile coordinates are 32-bit: a store of 2^31 - 128 tokens or more is scored in token segments of 2^30 tokens,
+    // one launch per segment (and query group), each with a tensor map that starts at the segment's first token.  A
+    // document belongs to the segment its first token lies in and may reach into the next one (documents are shorter
+    // than 2^30 tokens by contract).  Smaller stores are one segment.
+    const int64_t SEG = 1ll << 30;
+    const int64_t nseg = a.T < (1ll << 31) - BN ? 1 : (a.T + SEG - 1) / SEG;
     // one launch per group of Qg queries (up to 256 query rows): the store is streamed once per group
     const int Qeff = a.Q * pl.nparts;  // queries as the kernel sees them (32-token parts of long queries)
     float* dst = pl.nparts > 1 ? static_cast<float*>(a.workspace) : a.scores;
+    for (int64_t sg = 0; sg < nseg; ++sg)
     for (int q0 = 0; q0 < Qeff; q0 += pl.Qg) {
+        const int64_t tok0 = nseg == 1 ? 0 : sg * SEG;
+        const int64_t Tseg = nseg == 1 ? a.T : (a.T - tok0 < SEG ? a.T - tok0 : SEG);
+        int64_t map_rows = a.T - tok0;  // rows the segment's documents can touch: its own tokens + one more segment
+        if (map_rows > 2 * SEG - BN) map_rows = 2 * SEG - BN;
+        CUtensorMap map_docs = {};  // unused by the PQ decode variant
+        if (!pl.pqd && !cached_map_2d(&map_docs, di->device, a.dtype,
+                                      static_cast<const uint8_t*>(a.docs) + (size_t)tok0 * pl.p.row_bytes,
+                                      (uint64_t)map_rows, (uint64_t)a.d, (uint32_t)pl.p.kb_elems,
+                                      pl.pair ? BN / 2 : BN))  // a pair's CTAs load half a tile each
+            return TMS_ERR_CUDA;
+        // no more CTAs than 128-token tiles; one CTA per SM
+        int64_t grid = (Tseg + BN - 1) / BN;
+        if (grid > di->num_sms) grid = di->num_sms;
+        if (pl.pair) {  // one range per pair of CTAs (the two SMs of a TPC)
+            int64_t pairs = (Tseg + BN - 1) / BN;
+            if (pairs > di->num_sms / 2) pairs = di->num_sms / 2;
+            grid = 2 * pairs;
+        }
+#ifdef TMS_PROBES
+        if (const char* e = getenv("TMS_GRID")) { const int g = atoi(e); if (g > 0 && g < grid) grid = g; }
+        if (const char* e = getenv("TMS_NS")) { const int n = atoi(e); if (n > 0 && n < pl.p.NS) pl.p.NS = n; }
+#endif
         Params p = pl.p;
+        p.tok0 = tok0;
+        p.Tseg = Tseg;
+        p.seg_first = sg == 0;
+        p.seg_last = sg == nseg - 1;
         p.Q = Qeff - q0 < pl.Qg ? Qeff - q0 : pl.Qg;
         p.queries = static_cast<const uint8_t*>(a.queries) + (size_t)q0 * p.Nq * p.row_bytes;
         p.scores = dst + (int64_t)q0 * a.B;

@@ -44,7 +44,7 @@ def test_variant_used_is_a_pure_function_of_the_shape(Q, Nq, d, dtype, want):
 
 
 def test_variant_used_for_huge_and_degenerate_stores():
-    assert tms.tms_maxsim_variant_used(8, 32, 8, 1 << 20, (1 << 31) + 5, torch.bfloat16) == "simt"
+    assert tms.tms_maxsim_variant_used(8, 32, 8, 1 << 20, (1 << 31) + 5, torch.bfloat16) == "tcgen05"  # token segments
     assert tms.tms_maxsim_variant_used(8, 32, 128, 0, 0, torch.bfloat16) == "auto"
     assert tms.tms_maxsim_variant_used(8, 32, 128, 10, 0, torch.bfloat16) == "auto"
 

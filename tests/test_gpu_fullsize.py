@@ -139,3 +139,66 @@ def test_config4_fused_pq():
     assert float((got_d - f32_d).abs().max()) <= 0.25 * 2e-3 * Nq
     f32 = f32_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
     assert np.abs(f32 - ref).max() <= 2e-3 * Nq
+
+
+# ---- stores of 2^31 tokens and more: TMA coordinates are 32-bit, the library scores them in 2^30-token segments ---------
+
+def _huge_offsets(seed):
+    rng = np.random.default_rng(seed)
+    lens = rng.integers(1800, 2200, size=1_100_000).astype(np.int64)   # ~2.2e9 tokens > 2^31
+    lens[rng.choice(lens.size, size=2000, replace=False)] = 0           # empty documents, also near the segment cuts
+    return synth.offsets_from_lengths(lens)
+
+
+def _huge_sample(off, seed):
+    """Documents that straddle or touch the 2^30-token segment cuts (and their neighbours), plus a seeded sample."""
+    B, T = len(off) - 1, int(off[-1])
+    near = []
+    for cut in range(1 << 30, T, 1 << 30):
+        b = int(np.searchsorted(off, cut, side="right")) - 1            # the document that holds token `cut`
+        near += list(range(max(b - 4, 0), min(b + 5, B)))
+    rng = np.random.default_rng(seed)
+    return np.unique(np.concatenate([np.array(near, dtype=np.int64), rng.choice(B, size=300, replace=False), [0, B - 1]]))
+
+
+def test_dense_store_of_more_than_2_31_tokens():
+    off = _huge_offsets(seed=501)
+    B, T, Q, Nq, d = len(off) - 1, int(off[-1]), 4, 32, 8
+    assert T > (1 << 31)
+    assert tms.tms_maxsim_variant_used(Q, Nq, d, B, T, torch.bfloat16) == "tcgen05"
+    q = synth.unit_tokens(Q * Nq, d, torch.bfloat16, seed=502, device=DEV).view(Q, Nq, d)
+    D = synth.unit_tokens(T, d, torch.bfloat16, seed=503, device=DEV)   # 16-byte rows: 35 GB
+    off_d = torch.from_numpy(off).to(DEV)
+    got_d = tms.tms_maxsim(q, D, off_d)
+    torch.cuda.synchronize()
+    empty = torch.from_numpy(np.diff(off) == 0).to(DEV)
+    assert bool(torch.isneginf(got_d[:, empty]).all()) and bool(torch.isfinite(got_d[:, ~empty]).all())
+    sample = _huge_sample(off, seed=504)
+    sub, sub_off = gather_docs(D, off, sample)
+    ref = oracle.maxsim(q.cpu(), sub, sub_off)
+    got = got_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
+    inf = np.isneginf(ref)
+    assert np.array_equal(np.isneginf(got), inf)
+    assert np.abs(got[~inf] - ref[~inf]).max() <= tol(torch.bfloat16, Nq)
+    del D, got_d
+    torch.cuda.empty_cache()
+
+
+def test_pq_decode_store_of_more_than_2_31_tokens():
+    off = _huge_offsets(seed=511)
+    B, T, Q, Nq = len(off) - 1, int(off[-1]), 4, 32
+    q = synth.unit_tokens(Q * Nq, 128, torch.bfloat16, seed=512, device=DEV).view(Q, Nq, 128)
+    C = synth.pq_codebooks(16, 256, 8, seed=513)
+    codes = synth.pq_codes(T, 16, seed=514, device=DEV)                 # 35 GB of codes
+    off_d = torch.from_numpy(off).to(DEV)
+    got_d = tms.tms_pq_maxsim_decode(q, C.to(DEV), codes, off_d)
+    torch.cuda.synchronize()
+    sample = _huge_sample(off, seed=515)
+    sub, sub_off = gather_docs(codes, off, sample)
+    ref = oracle.pq_maxsim(q.cpu(), C, sub, sub_off)
+    got = got_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
+    inf = np.isneginf(ref)
+    assert np.array_equal(np.isneginf(got), inf)
+    assert np.abs(got[~inf] - ref[~inf]).max() <= 2e-3 * Nq
+    del codes, got_d
+    torch.cuda.empty_cache()
