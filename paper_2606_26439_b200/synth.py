@@ -122,3 +122,28 @@ def plant_relevant(queries: torch.Tensor, docs: torch.Tensor, offsets: np.ndarra
             t0 = int(offsets[ids[q, r]])
             docs[t0:t0 + Nq] = tok.to(docs.dtype).to(docs.device)
     return ids
+
+
+def plant_relevant_pq(queries: torch.Tensor, codebooks: torch.Tensor, codes: torch.Tensor, offsets: np.ndarray, seed: int,
+                      per_query: int = 32) -> np.ndarray:
+    """Planted PQ documents: document r of query q gets, as the codes of its first Nq - r tokens, the centroids closest (by
+    inner product) to query tokens 0 .. Nq - r - 1 in every sub-quantiser; the other tokens keep their random codes.
+    Each planted token lifts one query token's maximum far above what random codes reach, so the scores of a query's
+    planted documents fall by a clear step from rank to rank (the test checks the steps on the oracle's scores).
+    Modifies `codes` in place; returns ids[Q, per_query] in rank order.  per_query <= Nq."""
+    Q, Nq, d = queries.shape
+    M, K, dsub = codebooks.shape
+    if per_query > Nq:
+        raise ValueError("per_query <= Nq")
+    lengths = np.diff(offsets)
+    eligible = np.nonzero(lengths >= Nq)[0]
+    rng = np.random.default_rng(seed)
+    ids = rng.choice(eligible, size=Q * per_query, replace=False).reshape(Q, per_query)
+    qf = queries.detach().cpu().to(torch.float32).reshape(Q, Nq, M, dsub)
+    best = torch.einsum("qims,mks->qimk", qf, codebooks.detach().cpu().to(torch.float32)).argmax(dim=3)  # [Q, Nq, M]
+    for q in range(Q):
+        for r in range(per_query):
+            n = Nq - r
+            t0 = int(offsets[ids[q, r]])
+            codes[t0:t0 + n] = best[q, :n].to(torch.uint8).to(codes.device)
+    return ids

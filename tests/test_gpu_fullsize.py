@@ -111,6 +111,7 @@ def test_config4_fused_pq():
     q = synth.unit_tokens(Q * Nq, d, torch.bfloat16, seed=401, device=DEV).view(Q, Nq, d)
     C = synth.pq_codebooks(M, K, d // M, seed=402)
     codes = synth.pq_codes(int(off[-1]), M, seed=403, device=DEV, K=K)
+    ids_planted = synth.plant_relevant_pq(q, C, codes, off, seed=405)   # 32 planted documents per query, in rank order
     off_d = torch.from_numpy(off).to(DEV)
     lut = tms.tms_pq_build_lut(q, C.to(DEV))
     got_d = tms.tms_pq_maxsim(lut, codes, off_d)
@@ -118,9 +119,20 @@ def test_config4_fused_pq():
     torch.cuda.synchronize()
     assert torch.equal(got_d, again) and bool(torch.isfinite(got_d).all())
     rng = np.random.default_rng(404)
-    sample = np.unique(np.concatenate([rng.choice(B, size=1500, replace=False), [0, B - 1]]))
+    sample = np.unique(np.concatenate([rng.choice(B, size=1500, replace=False), ids_planted.reshape(-1), [0, B - 1]]))
     sub, sub_off = gather_docs(codes, off, sample)
     ref = oracle.pq_maxsim(q.cpu(), C, sub, sub_off)
+    # ranking over ALL 1,000,000 documents: the 16 best-planted documents of every query first, in order.  Their oracle
+    # scores step down by far more than the tolerance and stay far above every other sampled document (random ones and
+    # the documents planted for other queries), both checked here, so every kernel's top-16 is determined.
+    KTOP = 16
+    pos = {int(b): i for i, b in enumerate(sample)}
+    for qq in range(Q):
+        planted_ref = np.array([ref[qq, pos[int(b)]] for b in ids_planted[qq]])
+        assert np.all(planted_ref[:-1] - planted_ref[1:] > 4 * 2e-3 * Nq), "planted scores must step down clearly"
+        others = np.delete(ref[qq], [pos[int(b)] for b in ids_planted[qq, :KTOP]])
+        assert planted_ref[KTOP - 1] - others.max() > 1.0
+    assert np.array_equal(torch.topk(got_d, KTOP, dim=1).indices.cpu().numpy(), ids_planted[:, :KTOP])
     got = got_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
     err = np.abs(got - ref).max()
     assert err <= 2e-3 * Nq, f"max |dscore| = {err:.3e}"
@@ -136,6 +148,8 @@ def test_config4_fused_pq():
     # and what tms_pq_maxsim runs by default for this shape (fp16 table entries, a quarter of the tolerance at most)
     f32_d = tms.tms_pq_maxsim(lut, codes, off_d, variant="pq_smem")
     assert float((dec_d - f32_d).abs().max()) < 5e-4
+    for other in (dec_d, f32_d):
+        assert np.array_equal(torch.topk(other, KTOP, dim=1).indices.cpu().numpy(), ids_planted[:, :KTOP])
     assert float((got_d - f32_d).abs().max()) <= 0.25 * 2e-3 * Nq
     f32 = f32_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
     assert np.abs(f32 - ref).max() <= 2e-3 * Nq
