@@ -104,11 +104,12 @@ def test_all_documents_empty_pq_decode():
 
 # ---- host-buffer entry points against the oracle ---------------------------------------------------------------------------
 
-@pytest.mark.parametrize("Nq,dtype", [(32, torch.bfloat16), (64, torch.float16), (48, torch.bfloat16)])
-def test_host_entry_point_against_the_oracle(Nq, dtype):
+@pytest.mark.parametrize("Nq,dtype,Q,d", [(32, torch.bfloat16, 4, 128), (64, torch.float16, 4, 128), (48, torch.bfloat16, 4, 128),
+                                          (32, torch.bfloat16, 8, 512)])  # the last one: CTA pairs through the host call
+def test_host_entry_point_against_the_oracle(Nq, dtype, Q, d):
     lens = np.concatenate([RAGGED, synth.lognormal_lengths(1500, seed=7)])
     off = synth.offsets_from_lengths(lens)
-    Q, d, B = 4, 128, len(lens)
+    B = len(lens)
     q = synth.unit_tokens(Q * Nq, d, dtype, seed=35).view(Q, Nq, d)
     D = synth.unit_tokens(int(off[-1]), d, dtype, seed=36)
     scores = torch.empty((Q, B), dtype=torch.float32).pin_memory()
