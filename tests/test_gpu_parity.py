@@ -88,6 +88,16 @@ def test_degenerate_batches(variant, lens):
     assert_close(run_dense(q, D, off, variant), oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
 
 
+@pytest.mark.parametrize("lens", [[1], [128], [129], [7, 0], [0, 0, 3], [2000], [0, 5, 0, 0], [64, 64, 1]])
+@pytest.mark.parametrize("Nq", [32, 64])
+def test_degenerate_batches_as_cta_pairs(lens, Nq):
+    """The same corner cases through the CTA-pair kernel (d = 512, 256 query rows): one pair, one tile, empty documents;
+    Nq = 64 adds the two-part long-query scratch on top."""
+    off = synth.offsets_from_lengths(lens)
+    q, D = unit_case(8 if Nq == 32 else 5, Nq, 512, torch.float16, off, seed=19)
+    assert_close(run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off), tol(torch.float16, Nq))
+
+
 def test_all_single_token_documents():
     off = synth.uniform_offsets(5000, 1)
     q, D = unit_case(4, 32, 128, torch.float16, off, seed=11)
