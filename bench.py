@@ -477,6 +477,9 @@ def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):
         w = WORKLOADS[name]
         try:
             wl = Workload(name, w, w["B"], args.seed, dev, tms, reuse=prev)
+            torch.cuda.synchronize()
+            time.sleep(1.0)  # let the board's power controller settle after the previous workload (each config is timed
+            #                  on its own: a 0.4 ms kernel measured right behind a power-capped one inherits its clocks)
             step_ms, total_ms, clocks, launches = timed_region(wl, args.secondary_steps, 3, local_rank, sync_all, shard)
             r = roofline_of(wl, step_ms, total_ms, clocks, peaks)
             out[name] = {"ms_per_step": float(step_ms.mean()), "ms_min": float(step_ms.min()),
