@@ -805,6 +805,52 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             // region per tile, block-major -- both 64-dimension units of a block back to back (one accumulator switch
             // per tile, block 0's accumulator handed to the epilogue half a tile early), then the next block.
             const bool whole_tile = PQD && NS >= 4;
+            // ... and with only one tile's worth of stages (split bf16 operands: two 32 KB stages): still one region per
+            // tile, but unit-major, the issuing lane awaiting the second unit's stage itself and releasing each stage as
+            // soon as its MMAs are queued, so the next tile's decode starts as early as before.
+            const bool unit_major_tile = PQD && !whole_tile && nch == 2 && NS >= 2;
+            if (unit_major_tile) {
+                uint32_t s1 = s + 1, ph1 = ph;
+                if (s1 == NS) { s1 = 0; ph1 ^= 1; }
+                if (!early_full) mbar_wait(full0 + s * 8, ph);
+                if (!early_acc) mbar_wait(tempty0 + slot[0] * 8, tph[0] ^ 1);
+                tc_fence_after();
+                if (elect_one()) {
+#pragma unroll
+                    for (int ch = 0; ch < 2; ++ch) {
+                        if (ch == 1) {
+                            mbar_wait(full0 + s1 * 8, ph1);
+                            tc_fence_after();
+                        }
+                        const uint32_t b_lo = b_lo0 + (ch ? s1 : s) * (stage_bytes >> 4);
+#pragma unroll
+                        for (int mb = 0; mb < MB; ++mb) {
+                            if (ch == 0 && mb != 0) {
+                                mbar_wait(tempty0 + slot[mb] * 8, tph[mb] ^ 1);
+                                tc_fence_after();
+                            }
+                            const uint32_t d_tmem = acc0 + slot[mb] * BN;
+                            if (!skip) {
+#pragma unroll
+                                for (int kk = 0; kk < 4; ++kk) {
+                                    const uint64_t b_hi = ((uint64_t)DESC_HI << 32) | (b_lo + kk * 2);
+                                    const uint64_t b_lw = ((uint64_t)DESC_HI << 32) | (b_lo + (KB_TILE_BYTES >> 4) + kk * 2);
+                                    const uint32_t a_hi = a_col + ch * KB_WORDS + mb * a_mb_step + kk * 8;
+                                    tc_mma_ts(d_tmem, a_hi, b_hi, idesc, (ch != 0 || kk != 0) ? 1u : 0u);
+                                    if (!skip_blo) tc_mma_ts(d_tmem, a_hi, b_lw, idesc, 1u);
+                                    if (!skip_alo) tc_mma_ts(d_tmem, a_hi + a_lo_off, b_hi, idesc, 1u);
+                                }
+                            }
+                            if (ch == 1) tc_commit(tfull0 + (tq * MB + mb) * 8);  // accumulator -> epilogue
+                        }
+                        tc_commit(empty0 + (ch ? s1 : s) * 8);  // the stage goes back to the splitter warps
+                    }
+                    mbar_arrive(other_turn);  // the other issuer may start its tile
+                }
+                __syncwarp();
+                s += 2;
+                while (s >= NS) { s -= NS; ph ^= 1; }
+            }
             if (whole_tile) {
                 uint32_t s1 = s + 1, ph1 = ph;
                 if (s1 == NS) { s1 = 0; ph1 ^= 1; }
@@ -845,7 +891,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 s += 2;
                 while (s >= NS) { s -= NS; ph ^= 1; }
             }
-            for (uint32_t ch = 0; !whole_tile && ch < nch; ++ch) {
+            for (uint32_t ch = 0; !whole_tile && !unit_major_tile && ch < nch; ++ch) {
                 if (ch != 0 || !early_full) mbar_wait(full0 + s * 8, ph);
                 const uint32_t b_lo = b_lo0 + s * (stage_bytes >> 4);
                 const bool last_chunk = ch == nch - 1;
