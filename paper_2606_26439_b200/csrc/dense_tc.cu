@@ -808,7 +808,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             // ... and with only one tile's worth of stages (split bf16 operands: two 32 KB stages): still one region per
             // tile, but unit-major, the issuing lane awaiting the second unit's stage itself and releasing each stage as
             // soon as its MMAs are queued, so the next tile's decode starts as early as before.
-            const bool unit_major_tile = PQD && !whole_tile && nch == 2 && NS >= 2;
+            const bool unit_major_tile = F32 && !whole_tile && nch == 2 && NS >= 2;
             // CTA pairs (one query block, d > 256: three to six 256-byte chunks per tile): one region per tile as well -- the
             // issuing lane awaits each later chunk's stage itself, so a tile's 24-48 MMAs are queued without the per-region
             // overhead between every eight of them (ncu: tensor pipe 78 % -> see profiles).
