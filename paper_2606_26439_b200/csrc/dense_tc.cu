@@ -339,8 +339,10 @@ __device__ void warp_lower_bound2(const int64_t* __restrict__ offsets, int64_t B
     val_b = bb ? xb_f : b.val;
 }
 
-struct SegInfo {
+struct __align__(16) SegInfo {
     uint32_t mask[4];     // bit c set: column c of the tile is the last token of a (non-empty) document
+    uint32_t ord0;        // ordinal (see DOCRING) of the first document that ends in this tile
+    uint32_t pad[3];
 };
 // The CTA's non-empty documents are numbered in order ("ordinals"); DOCRING maps ordinal -> document index relative to
 // the CTA's first document.  The segmenter is at most NSEG tiles (<= 128 documents each) ahead of the slowest epilogue
@@ -596,9 +598,13 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
 // A stage is shared state: it is refilled only when BOTH CTAs' tensor pipes have read it (the `empty` barriers count two
 // arrivals, each CTA's tcgen05.commit is multicast to both).  Everything else -- MMA issue, segmenter, epilogue, max->sum
 // -- is per CTA and unchanged (Thm 1's ceil(Nq/BQ) factor stays 1).
-template <int MB, int KBS, bool F32, bool PQD, int NSET, bool PAIR = false>
+// ALT (with NSET = 2): the two epilogue sets take alternate TILES instead of column halves -- every warp reduces whole
+// 128-column rows but only of every other tile, so it has two tile periods for a tile's segmented reduction; the running
+// maximum crosses tiles through the same mailbox (one hop per tile).
+template <int MB, int KBS, bool F32, bool PQD, int NSET, bool PAIR = false, bool ALT = false>
 __global__ void __launch_bounds__(128 + NSET * 128 * MB + (F32 ? 128 : 0), 1)
 dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
+    static_assert(!ALT || (NSET == 2 && !F32 && !PAIR), "alternate-tile epilogue sets: two sets, 16-bit inputs");
     static_assert(!PAIR || (MB == 1 && !F32 && !PQD), "CTA pairs: one query block per CTA, 16-bit inputs");
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // 128-byte-swizzled operand tiles need 1024-byte alignment in the shared window
@@ -642,9 +648,9 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         if (lane == 0) {
             for (int s = 0; s < p.NS; ++s) { mbar_init(smem_u32(full + s), F32 ? 4 : 1); mbar_init(smem_u32(empty + s), PAIR ? 2 : 1); }
             for (int s = 0; s < 8; ++s) mbar_init(smem_u32(tfull + s), 1);
-            for (int s = 0; s < MAX_ACC; ++s) mbar_init(smem_u32(tempty + s), 4 * NSET);
+            for (int s = 0; s < MAX_ACC; ++s) mbar_init(smem_u32(tempty + s), 4 * (ALT ? 1 : NSET));
             for (int s = 0; s < MAX_RAW; ++s) { mbar_init(smem_u32(rfull + s), 1); mbar_init(smem_u32(rempty + s), 4); }
-            for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), NSET * n_epi_warps); }
+            for (int s = 0; s < NSEG; ++s) { mbar_init(smem_u32(sfull + s), 1); mbar_init(smem_u32(sempty + s), (ALT ? 1 : NSET) * n_epi_warps); }
             mbar_init(smem_u32(aready), n_epi_warps);
             mbar_init(smem_u32(turn), 1);
             mbar_init(smem_u32(turn + 1), 1);
@@ -1084,8 +1090,8 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 e_nxt = load_ends(wb + 32);
                 consumed = 0;
             }
+            if (lane == 0) { seg[g].mask[0] = m0; seg[g].mask[1] = m1; seg[g].mask[2] = m2; seg[g].mask[3] = m3; seg[g].ord0 = ord; }
             ord += nseg;
-            if (lane == 0) { seg[g].mask[0] = m0; seg[g].mask[1] = m1; seg[g].mask[2] = m2; seg[g].mask[3] = m3; }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sfull + g));
         }
@@ -1268,7 +1274,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         const bool skip_math = PROBE(p, 1);
         const int64_t B = p.B;
         const uint32_t ring = smem_u32(docring);
-        const bool frees_stage = !F32 && !PAIR && nchunks == 1 && set == 0 && ew == 4 * (MB - 1);  // see the MMA warps
+        const bool frees_stage = !F32 && !PAIR && nchunks == 1 && (ALT || set == 0) && ew == 4 * (MB - 1);  // see the MMA warps
 
         // Two sets (16-bit inputs): set 0 reduces columns 0..63 of every tile, set 1 columns 64..127.  A tcgen05.ld
         // blocks the issuing warp until its data are in registers (measured: two loads "in flight" from one warp take
@@ -1303,18 +1309,23 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
         };
         const uint32_t nacc = (uint32_t)p.NACC, NS = (uint32_t)p.NS;
         const uint32_t acc0 = lane_addr + (uint32_t)p.acc_col0;
-        uint32_t slot = (uint32_t)mb, g = 0, gph = 0, rs = 0;
+        // ring positions of this warp's first tile (ALT: set s starts at tile s and advances two tiles at a time)
+        constexpr uint32_t TSTEP = ALT ? 2u : 1u;
+        uint32_t slot = (uint32_t)mb + (ALT ? (uint32_t)(set * MB) : 0u), g = ALT ? (uint32_t)set : 0u, gph = 0, rs = ALT ? (uint32_t)set : 0u;
+        while (slot >= nacc) slot -= nacc;
+        while (rs >= NS) rs -= NS;
         uint32_t ord_tile = 0;  // (two sets) non-empty documents that ended in earlier tiles
         const bool tr = quad == 0 && (set == 0 || mb == 0);  // (probe builds) the warps whose clocks are traced
         const int trole = set == 0 ? 2 + mb : 0;
         const int nt = (int)ntiles;
-        for (int t = 0; t < nt; ++t) {
+        for (int t = ALT ? set : 0; t < nt; t += (int)TSTEP) {
             if (tr) TRACED(trole, t, 0);
             mbar_wait(smem_u32(tfull + (uint32_t)(t & 3) * MB + mb), (uint32_t)(t >> 2) & 1u);
             tc_fence_after();
             if (frees_stage) {  // the tile's only stage has been read by the tensor pipe: back to the producer
                 if (lane == 0) mbar_arrive(smem_u32(empty + rs));
-                if (++rs == NS) rs = 0;
+                rs += TSTEP;
+                while (rs >= NS) rs -= NS;
             }
             if (tr) TRACED(trole, t, 1);
             const uint32_t taddr = acc0 + slot * BN;
@@ -1341,13 +1352,15 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                 process32(v + 32, mask.w, st, pend, ring, out, B, cfg, lane, skip_math, resolve);
             } else {
                 float v[32];
-                constexpr int NW = 4 / NSET;                   // 32-column words of a tile that are this warp's
-                const uint32_t c0 = (uint32_t)set * (NW * 32);  // its first column
+                constexpr int NW = ALT ? 4 : 4 / NSET;         // 32-column words of a tile that are this warp's
+                const uint32_t c0 = ALT ? 0u : (uint32_t)set * (NW * 32);  // its first column
                 tmem_ld32(taddr + c0, v);
                 mbar_wait(smem_u32(sfull + g), gph);
                 const uint4 mask = *reinterpret_cast<const uint4*>(seg[g].mask);
                 const uint32_t wds[4] = {mask.x, mask.y, mask.z, mask.w};
-                if (NSET == 2) {  // ordinal of the first document that ends in this warp's columns
+                if (ALT) {  // ordinal of the first document that ends in this tile: the segmenter's running count
+                    st.ord = seg[g].ord0;
+                } else if (NSET == 2) {  // ordinal of the first document that ends in this warp's columns
                     const uint32_t lo = __popc(mask.x) + __popc(mask.y);
                     st.ord = ord_tile + (set ? lo : 0);
                     ord_tile += lo + __popc(mask.z) + __popc(mask.w);
@@ -1367,11 +1380,11 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
                         if (lane == 0) mbar_arrive(smem_u32(tempty + slot));
                     }
                     if (tr) TRACED(trole, t, 2 + i);
-                    process32(v, wds[(NSET == 2 && set ? 2 : 0) + i], st, pend, ring, out, B, cfg, lane, skip_math, resolve);
+                    process32(v, wds[(NSET == 2 && !ALT && set ? 2 : 0) + i], st, pend, ring, out, B, cfg, lane, skip_math, resolve);
                 }
                 if constexpr (NSET == 2) {
                     if (st.unresolved) resolve();
-                    if (set == 0 || t + 1 < nt) {  // this range's carry -> the other set
+                    if ((!ALT && set == 0) || t + 1 < nt) {  // this range's carry -> the other set
                         sts_f32(mail_out, st.m);
                         __syncwarp();
                         if (lane == 0) mbar_arrive(carry_out);
@@ -1381,9 +1394,10 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(sempty + g));
-            slot += MB;
-            if (slot >= nacc) slot -= nacc;
-            if (++g == NSEG) { g = 0; gph ^= 1; }
+            slot += MB * TSTEP;
+            while (slot >= nacc) slot -= nacc;
+            g += TSTEP;
+            if (g >= NSEG) { g -= NSEG; gph ^= 1; }
         }
         if (st.np) drain(pend, st.np, out, B, cfg, ring, lane);
     }
@@ -1523,6 +1537,7 @@ struct Plan {
     int Qg;             // queries per launch
     int nset;           // epilogue warp sets
     bool pair;          // clusters of two CTAs, one query block each, document tiles multicast to both
+    bool alt;           // two epilogue sets on alternate tiles instead of column halves
     uint32_t smem_bytes;
 };
 
@@ -1603,8 +1618,14 @@ bool plan(const DenseArgs& a, Plan& pl) {
     // two epilogue sets when documents are short on average (< 100 tokens: most tiles then hold a document boundary
     // or several, and the segmented reduction binds), measured on config 3 (mean 72 tokens) against config 2 (128)
     pl.nset = (!f32 && a.T < 100 * a.B) ? 2 : 1;
+    // one query block and long documents: a lone epilogue warp per scheduler cannot keep up with the stream (TMEM loads
+    // and the reduction are one latency chain: ~870 clk per tile against 634 clk of HBM time at d = 64), so two sets take
+    // alternate tiles (measured: c4-d64 -24 %, c2-q4 -6 %; with two blocks or short documents it does not pay)
+    pl.alt = !f32 && !pair && MB == 1 && pl.nset == 1;
+    if (pl.alt) pl.nset = 2;
 #ifdef TMS_PROBES
     if (const char* e = getenv("TMS_NSET")) { const int n = atoi(e); if (!f32 && (n == 1 || n == 2)) pl.nset = n; }
+    if (const char* e = getenv("TMS_ALT")) { pl.alt = !f32 && !pair && atoi(e) != 0; if (pl.alt) pl.nset = 2; else if (MB == 1 && a.T >= 100 * a.B) pl.nset = 1; }
 #endif
     pl.KBS = f32 ? 2 : ((NKB % 2 == 0) ? 2 : 1);
     const uint32_t fixed = fixed_smem(MB, pl.nset);
@@ -1671,6 +1692,9 @@ int launch_dense_tc(const DenseArgs& a) {
     else if (pl.pair) {
         if (pl.nset == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 1, true> : dense_tc_kernel<1, 2, false, false, 1, true>;
         else kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 2, true> : dense_tc_kernel<1, 2, false, false, 2, true>;
+    } else if (pl.alt) {
+        if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 2, false, true> : dense_tc_kernel<1, 2, false, false, 2, false, true>;
+        else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 2, false, true> : dense_tc_kernel<2, 2, false, false, 2, false, true>;
     } else if (pl.nset == 1) {
         if (pl.MB == 1) kern = pl.KBS == 1 ? dense_tc_kernel<1, 1, false, false, 1> : dense_tc_kernel<1, 2, false, false, 1>;
         else kern = pl.KBS == 1 ? dense_tc_kernel<2, 1, false, false, 1> : dense_tc_kernel<2, 2, false, false, 1>;
