@@ -46,7 +46,8 @@ typedef enum {
     TMS_ERR_UNSUPPORTED = 2, /* shape / dtype / device outside what this build implements      */
     TMS_ERR_ALIGNMENT = 3,   /* a pointer or row pitch is not 16-byte aligned                  */
     TMS_ERR_WORKSPACE = 4,   /* workspace is NULL or smaller than the *_workspace_bytes() size  */
-    TMS_ERR_CUDA = 5         /* a CUDA runtime / driver call failed (launch, copy, attribute)  */
+    TMS_ERR_CUDA = 5,        /* a CUDA runtime / driver call failed (launch, copy, attribute)  */
+    TMS_ERR_STATIC_SCRATCH = 6 /* tms_topk_static: the shape needs more scratch than the built-in buffer holds */
 } tms_status;
 
 /* Storage dtype of query and document embeddings.  Arithmetic: products of the stored values,
@@ -224,6 +225,44 @@ int tms_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_
              size_t workspace_bytes, void* stream);
 
 size_t tms_topk_workspace_bytes(int Q, int64_t B, int k);
+
+/*
+ * tms_topk without a workspace argument and without any allocation -- the one entry point of this library for callers
+ * that have no device memory to give and no way to get some:
+ *   - a process whose HBM was handed, whole, to another component's pool at start-up (an inference server's KV-cache
+ *     arena, a framework's caching allocator run at its memory limit), so cudaMalloc would return out-of-memory;
+ *   - a plug-in or callback that runs where the host forbids calls that synchronise the device or take the driver's
+ *     allocation lock (cudaMalloc and cudaFree do both), e.g. a scoring hook inside a latency-bound serving loop;
+ *   - a plain C caller with no allocator of its own that wants one call and no buffer whose lifetime it must manage.
+ * Everything else in the library takes its scratch through `workspace`; this call takes none.  The selection levels'
+ * two key buffers live instead in a fixed array inside the library's device image:
+ *
+ *     TMS_TOPK_STATIC_SCRATCH_BYTES = 4 MiB, held by EVERY GPU that loads libtms.so from load until process exit,
+ *     whether or not this function is ever called.
+ *
+ * Result, order, tie rule and argument meaning are exactly tms_topk's (same kernels, same launch sequence: the outputs
+ * are bit-identical).  The caller still owns and passes `scores`, `values` and `indices`.
+ * Limit: shapes with tms_topk_workspace_bytes(Q, B, k) > TMS_TOPK_STATIC_SCRATCH_BYTES are rejected with
+ * TMS_ERR_STATIC_SCRATCH before anything is launched (the need is 16 * Q * ceil(B/4096) * k bytes for B > 4096, else
+ * 0: Q=8, k=100 fits up to B = 1.3M documents; Q=1, k=1024 up to B = 1.0M; Q=8, k=1024 up to B = 131K).  Such shapes
+ * need tms_topk with a caller-provided workspace; nothing falls back silently.
+ * First call on each device: the library asks the CUDA runtime for the array's address on the current device (once
+ * per device, cached; the device current at the time of the call is the one used).  That look-up can make the runtime
+ * load the library's device code onto that GPU, so make the first call on a device during start-up, outside any stream
+ * capture.  Later calls do no set-up.
+ * Sharing: there is ONE array per GPU and every call on that GPU uses it.  It keeps whatever the last call left there;
+ * no call depends on its contents (every key a level reads was written by the level before it, in the same call), so
+ * nothing needs clearing between calls.  Two calls whose kernels can overlap on the GPU -- different streams without
+ * an event between them, or two host threads -- race on the array and both results are garbage: keep all
+ * tms_topk_static calls of a device on one stream or order them with events.
+ * Makes no CUDA allocation and calls no allocating library routine.  Errors: as tms_topk, plus TMS_ERR_STATIC_SCRATCH;
+ * TMS_ERR_CUDA if the address look-up fails.
+ */
+#define TMS_TOPK_STATIC_SCRATCH_BYTES (4u << 20)
+int tms_topk_static(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* stream);
+
+/* = TMS_TOPK_STATIC_SCRATCH_BYTES of the loaded library (for callers that cannot see this header). */
+size_t tms_topk_static_scratch_bytes(void);
 
 /*
  * k-way merge of per-shard top-k lists -- the step after data-parallel scoring ("only a final concatenation of

@@ -250,6 +250,22 @@ size_t tms_topk_workspace_bytes(int Q, int64_t B, int k) {
     return topk_workspace_bytes(Q, B, k);
 }
 
+// tms_topk for callers that cannot provide a workspace: same checks, scratch in the library's built-in device array.
+// No cudaMalloc / cudaFree / allocating library routine anywhere below this call.
+int tms_topk_static(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* stream) {
+    if (Q <= 0 || B <= 0 || k <= 0 || !scores || !values || !indices) return TMS_ERR_INVALID_ARG;
+    if (k > B) return TMS_ERR_INVALID_ARG;
+    if (k > 1024 || B > (1ll << 31) || Q > 65535) return TMS_ERR_UNSUPPORTED;
+    if ((reinterpret_cast<uintptr_t>(scores) & 3u) || (reinterpret_cast<uintptr_t>(values) & 3u) ||
+        (reinterpret_cast<uintptr_t>(indices) & 7u))
+        return TMS_ERR_ALIGNMENT;
+    if (topk_workspace_bytes(Q, B, k) > (size_t)TMS_TOPK_STATIC_SCRATCH_BYTES) return TMS_ERR_STATIC_SCRATCH;
+    if (!device_info()) return TMS_ERR_CUDA;
+    return launch_topk_static(scores, Q, B, k, values, indices, static_cast<cudaStream_t>(stream));
+}
+
+size_t tms_topk_static_scratch_bytes(void) { return (size_t)TMS_TOPK_STATIC_SCRATCH_BYTES; }
+
 int tms_topk_merge(const float* values, const int64_t* indices, const int64_t* shard_base, int G, int Q, int k_in, int k,
                    float* out_values, int64_t* out_indices, void* workspace, size_t workspace_bytes, void* stream) {
     if (G <= 0 || Q <= 0 || k_in <= 0 || k <= 0 || !values || !indices || !shard_base || !out_values || !out_indices)
@@ -284,6 +300,9 @@ const char* tms_status_string(int status) {
         case TMS_ERR_ALIGNMENT: return "pointer or row pitch not 16-byte aligned";
         case TMS_ERR_WORKSPACE: return "workspace missing or too small";
         case TMS_ERR_CUDA: return "CUDA error";
+        case TMS_ERR_STATIC_SCRATCH:
+            return "shape needs more scratch than the library's built-in static buffer holds "
+                   "(tms_topk_workspace_bytes > TMS_TOPK_STATIC_SCRATCH_BYTES): use tms_topk with a workspace";
         default: return "unknown status";
     }
 }

@@ -74,6 +74,10 @@ size_t topk_workspace_bytes(int Q, int64_t B, int k);
 int launch_topk(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices, void* workspace,
                 cudaStream_t stream);
 
+// the same with the key buffers in the library's built-in device array (tms_topk_static)
+int launch_topk_static(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices,
+                       cudaStream_t stream);
+
 size_t topk_merge_workspace_bytes(int G, int Q, int k_in, int k);
 int launch_topk_merge(const float* values, const int64_t* indices, const int64_t* shard_base, int G, int Q, int k_in,
                       int k, float* out_values, int64_t* out_indices, void* workspace, cudaStream_t stream);

@@ -7,7 +7,16 @@
 // scores into chunks of 4096, sorts each chunk in shared memory (bitonic, descending) and keeps its k best keys;
 // the following levels do the same on the surviving keys until one chunk is left, whose k best are unpacked into
 // values[Q, k] and indices[Q, k].  With k <= 1024 every level shrinks the list at least four-fold.
+#include <mutex>
+
 #include "tms_internal.h"
+
+// Built-in scratch of tms_topk_static (include/tms.h): the two ping-pong key buffers of the selection levels, for
+// callers that have no device memory to hand over as a workspace.  It is part of the library's device image, so every
+// GPU that loads libtms.so carries these TMS_TOPK_STATIC_SCRATCH_BYTES until the process exits, whether or not
+// tms_topk_static is ever called.  On the host this name is only a handle for the runtime's symbol lookup -- it is NOT
+// a device address and must never be passed to a kernel; static_scratch() below asks the runtime for the real one.
+static __device__ __align__(256) unsigned char g_tms_topk_static_scratch[TMS_TOPK_STATIC_SCRATCH_BYTES];
 
 namespace tms {
 namespace {
@@ -151,6 +160,48 @@ int launch_topk_merge(const float* values, const int64_t* indices, const int64_t
     const int64_t pitch1 = chunks_of(n) * k;
     uint64_t* b0 = keys + (size_t)total;
     return run_levels(nullptr, keys, n, n, Q, k, b0, b0 + (size_t)Q * pitch1, pitch1, out_values, out_indices, stream);
+}
+
+// Device address of g_tms_topk_static_scratch on the CURRENT device, looked up once per device (the array exists once
+// per GPU, at a different address on each) and cached.  The lookup may make the runtime load the library's device image
+// onto that GPU, which is why the first tms_topk_static call on a device belongs outside any stream capture.
+static int static_scratch(uint64_t** out) {
+    constexpr int MAX_DEVICES = 64;
+    static std::mutex mu;
+    static uint64_t* cached[MAX_DEVICES] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) {
+        cudaGetLastError();
+        return TMS_ERR_CUDA;
+    }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!cached[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_tms_topk_static_scratch) != cudaSuccess || !p) {
+            cudaGetLastError();
+            return TMS_ERR_CUDA;
+        }
+        cached[dev] = static_cast<uint64_t*>(p);
+    }
+    *out = cached[dev];
+    return TMS_OK;
+}
+
+// tms_topk with the key buffers in the built-in array: same kernels, same launch sequence, no allocation of any kind.
+// Nothing in the array has to start from a known state: every level writes all nch*k keys of its output buffer
+// (chunks with fewer than k live keys pad with the all-zero key) before the next level reads exactly those.
+int launch_topk_static(const float* scores, int Q, int64_t B, int k, float* values, int64_t* indices,
+                       cudaStream_t stream) {
+    const size_t need = topk_workspace_bytes(Q, B, k);
+    if (need > (size_t)TMS_TOPK_STATIC_SCRATCH_BYTES) return TMS_ERR_STATIC_SCRATCH;
+    uint64_t* b0 = nullptr;
+    if (need) {
+        const int st = static_scratch(&b0);
+        if (st != TMS_OK) return st;
+    }
+    const int64_t pitch1 = chunks_of(B) * k;
+    return run_levels(scores, nullptr, B, B, Q, k, b0, b0 ? b0 + (size_t)Q * pitch1 : nullptr, pitch1, values, indices,
+                      stream);
 }
 
 }  // namespace tms

@@ -41,6 +41,8 @@ SIGNATURES = {
     "tms_pq_maxsim_host_workspace_min_bytes": (_sz, [_i, _i, _i, _i, _i, _i, _i64]),
     "tms_topk": (_i, [_vp, _i, _i64, _i, _vp, _vp, _vp, _sz, _vp]),
     "tms_topk_workspace_bytes": (_sz, [_i, _i64, _i]),
+    "tms_topk_static": (_i, [_vp, _i, _i64, _i, _vp, _vp, _vp]),
+    "tms_topk_static_scratch_bytes": (_sz, []),
     "tms_topk_merge": (_i, [_vp, _vp, _vp, _i, _i, _i, _i, _vp, _vp, _vp, _sz, _vp]),
     "tms_topk_merge_workspace_bytes": (_sz, [_i, _i, _i, _i]),
     "tms_launch_count": (_u64, []),
@@ -221,6 +223,33 @@ def tms_topk(scores: torch.Tensor, k: int, values: torch.Tensor | None = None, i
     st = lib.tms_topk(_dev(scores, "scores"), Q, B, k, _dev(values, "values"), _dev(indices, "indices"), ws_ptr, ws_len,
                       _stream(stream))
     _check(st, "tms_topk")
+    return values, indices
+
+
+def tms_topk_static_scratch_bytes() -> int:
+    """Size of the library's built-in top-k scratch array (TMS_TOPK_STATIC_SCRATCH_BYTES)."""
+    return int(load().tms_topk_static_scratch_bytes())
+
+
+def tms_topk_static(scores: torch.Tensor, k: int, values: torch.Tensor | None = None,
+                    indices: torch.Tensor | None = None, stream=None):
+    """tms_topk for callers that cannot allocate device memory (include/tms.h: tms_topk_static): same result, bit for
+    bit, but the scratch is a fixed 4 MiB array inside the library instead of a workspace, and the library allocates
+    nothing.  Pass `values` (fp32 [Q,k]) and `indices` (int64 [Q,k]) to keep this wrapper from allocating them too.
+    Shapes whose scratch exceeds the array raise (status 6) -- use tms_topk with a workspace for those.  All calls on
+    one GPU share the array: keep them on one stream, and make the first call on a device outside stream capture."""
+    Q, B = scores.shape
+    if scores.dtype != torch.float32:
+        raise ValueError("scores must be fp32 [Q,B]")
+    if values is None:
+        values = torch.empty((Q, k), dtype=torch.float32, device=scores.device)
+    if indices is None:
+        indices = torch.empty((Q, k), dtype=torch.int64, device=scores.device)
+    if values.shape != (Q, k) or values.dtype != torch.float32 or indices.shape != (Q, k) or indices.dtype != torch.int64:
+        raise ValueError("values must be fp32 [Q,k] and indices int64 [Q,k]")
+    st = load().tms_topk_static(_dev(scores, "scores"), Q, B, k, _dev(values, "values"), _dev(indices, "indices"),
+                                _stream(stream))
+    _check(st, "tms_topk_static")
     return values, indices
 
 
