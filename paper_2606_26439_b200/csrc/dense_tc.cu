@@ -123,8 +123,9 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// The suspend-time hint lets the hardware park the warp until the phase completes (or the hint expires) instead of
-// returning early: a warp that spins on try_wait takes issue slots from the working warps of its sub-partition.
+// try_wait (unlike test_wait) lets the hardware suspend the warp until the phase completes or an implementation time
+// limit expires, instead of returning at once: a warp that spins takes issue slots from the working warps of its
+// sub-partition.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
@@ -135,7 +136,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "bra LAB_WAIT;\n"
         "DONE:\n"
         "}\n" ::"r"(bar),
-        "r"(parity), "r"(0x989680u)
+        "r"(parity)
         : "memory");
 }
 // non-blocking: has the phase with this parity completed?
@@ -345,8 +346,12 @@ struct __align__(16) SegInfo {
     uint32_t pad[3];
 };
 // The CTA's non-empty documents are numbered in order ("ordinals"); DOCRING maps ordinal -> document index relative to
-// the CTA's first document.  The segmenter is at most NSEG tiles (<= 128 documents each) ahead of the slowest epilogue
-// warp, which holds at most PEND parked documents plus its current tile's: 16 + 128 + 512 < DOCRING entries are live.
+// the CTA's first document.  An entry is read when its document is PARKED, i.e. while the epilogue warp still holds the
+// tile the document ends in: the segmenter is at most NSEG tiles (<= 128 documents each) ahead of the slowest epilogue
+// warp, so at most 128 + (NSEG - 1) * 128 = 512 < DOCRING ordinals separate the entry from the newest one written.
+// (Reading it later, when the park buffer is drained, would not be safe: ordinals count ALL of the CTA's documents,
+// while a warp of two epilogue sets parks only those that end in its own columns / tiles, so a parked document can
+// wait while far more than DOCRING ordinals go by.)
 constexpr uint32_t DOCRING = 1024;
 
 // ---- epilogue helpers ------------------------------------------------------------------------------------------
@@ -385,11 +390,12 @@ __device__ __forceinline__ float lds_f32(uint32_t addr) {
 }
 
 // A document's last token has been folded in: row `lane` parks its maximum in slot np of the warp's buffer.
-// pend: shared-window byte address of this warp's park buffer ([PEND][PEND_PITCH] floats, then PEND document ordinals).
+// pend: shared-window byte address of this warp's park buffer ([PEND][PEND_PITCH] floats, then PEND document indices,
+// relative to the CTA's first document: the ordinal is resolved through DOCRING here, while its entry is live).
 constexpr uint32_t PEND_IDS = PEND * PEND_PITCH * 4;  // byte offset of the ids inside a warp's park buffer
-__device__ __forceinline__ void park(float m, uint32_t ord, uint32_t np, uint32_t pend, int lane) {
+__device__ __forceinline__ void park(float m, uint32_t ord, uint32_t np, uint32_t pend, uint32_t ring, int lane) {
     sts_f32(pend + (np * PEND_PITCH + lane) * 4, m);
-    if (lane == 0) sts_u32(pend + PEND_IDS + np * 4, ord);
+    if (lane == 0) sts_u32(pend + PEND_IDS + np * 4, lds_u32(ring + (ord & (DOCRING - 1)) * 4));
 }
 
 // max -> sum (Eq. 1) for the np parked documents.  Rows that no query token owns hold zero query vectors, so their
@@ -398,7 +404,7 @@ __device__ __forceinline__ void park(float m, uint32_t ord, uint32_t np, uint32_
 //   Nq_pad = 32 (one query per warp): lanes j and j+16 add rows 0..15 / 16..31 of parked document j with four
 //   16-byte loads each, in four interleaved partial sums, and lane j stores the score.
 //   Nq_pad < 32: one lane per (document, query of this warp), rows added in ascending order.
-__device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64_t B, uint32_t cfg, uint32_t ring, int lane) {
+__device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64_t B, uint32_t cfg, int lane) {
     const uint32_t Nq_pad = (cfg >> 6) & 63u, nvalid = (cfg >> 12) & 63u;
     __syncwarp();
     if (Nq_pad == 32) {
@@ -409,7 +415,7 @@ __device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64
         const float a2 = (x0.z + x1.z) + (x2.z + x3.z), a3 = (x0.w + x1.w) + (x2.w + x3.w);
         float acc = (a0 + a1) + (a2 + a3);
         acc += __shfl_xor_sync(0xffffffffu, acc, 16);
-        if (h == 0 && j < np && nvalid) out[lds_u32(ring + (lds_u32(pend + PEND_IDS + j * 4) & (DOCRING - 1)) * 4)] = acc;
+        if (h == 0 && j < np && nvalid) out[lds_u32(pend + PEND_IDS + j * 4)] = acc;
     } else {
         const uint32_t nsub = 32u / Nq_pad;
         for (uint32_t u = lane; u < np * nsub; u += 32) {
@@ -418,7 +424,7 @@ __device__ __noinline__ void drain(uint32_t pend, uint32_t np, float* out, int64
                 const uint32_t p = pend + (slot * PEND_PITCH + sub * Nq_pad) * 4;
                 float acc = lds_f32(p);
                 for (uint32_t r = 1; r < Nq_pad; ++r) acc += lds_f32(p + r * 4);
-                out[(int64_t)sub * B + lds_u32(ring + (lds_u32(pend + PEND_IDS + slot * 4) & (DOCRING - 1)) * 4)] = acc;
+                out[(int64_t)sub * B + lds_u32(pend + PEND_IDS + slot * 4)] = acc;
             }
         }
     }
@@ -447,12 +453,12 @@ struct EpiState {
     float head;
 };
 // a document closes with row maximum `value`
-__device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pend, int lane) {
+__device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pend, uint32_t ring, int lane) {
     if (s.unresolved && s.first == NONE) {
         s.first = s.np;
         s.head = value;
     }
-    park(value, s.ord, s.np, pend, lane);
+    park(value, s.ord, s.np, pend, ring, lane);
     ++s.ord;
     ++s.np;
 }
@@ -462,13 +468,13 @@ __device__ __forceinline__ void close_doc(float value, EpiState& s, uint32_t pen
 // one compact copy keeps the epilogue's hot loop short.  The caller has made sure the buffer has room.
 __device__ __noinline__ float epi_chunk_slow(float x0, float x1, float x2, float x3, float x4, float x5, float x6,
                                              float x7, uint32_t byte, float m, uint32_t ord, uint32_t np, uint32_t pend,
-                                             int lane) {
+                                             uint32_t ring, int lane) {
     const float x[8] = {x0, x1, x2, x3, x4, x5, x6, x7};
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         m = fmaxf(m, x[c]);
         if (byte & (1u << c)) {
-            park(m, ord, np, pend, lane);
+            park(m, ord, np, pend, ring, lane);
             ++ord;
             ++np;
             m = -INFINITY;  // Alg. 3 line 4 for the next document
@@ -526,17 +532,17 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
     if (w == 0x80000000u) {  // the word's last column (uniform 128-token documents)
         if (s.np == PEND) {
             if (s.unresolved) resolve();
-            drain(pend, s.np, out, B, cfg, ring, lane);
+            drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
-        close_doc(max33(s.m, v), s, pend, lane);
+        close_doc(max33(s.m, v), s, pend, ring, lane);
         s.m = -INFINITY;  // Alg. 3 line 4 for the next document
         return;
     }
     if ((w & (w - 1)) == 0) {
         if (s.np == PEND) {
             if (s.unresolved) resolve();
-            drain(pend, s.np, out, B, cfg, ring, lane);
+            drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
         float closed, open;
@@ -548,7 +554,7 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
             if (e < 24) split_word<2>(v, e8, s.m, closed, open);
             else split_word<3>(v, e8, s.m, closed, open);
         }
-        close_doc(closed, s, pend, lane);
+        close_doc(closed, s, pend, ring, lane);
         s.m = open;
         return;
     }
@@ -562,11 +568,11 @@ __device__ __forceinline__ void process32(const float* v, uint32_t w, EpiState& 
         }
         if (s.np + __popc(byte) > PEND) {  // room for the documents that end in this chunk
             if (s.unresolved) resolve();
-            drain(pend, s.np, out, B, cfg, ring, lane);
+            drain(pend, s.np, out, B, cfg, lane);
             s.np = 0;
         }
         const bool rec = s.unresolved && s.first == NONE;
-        s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.ord, s.np, pend, lane);
+        s.m = epi_chunk_slow(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7], byte, s.m, s.ord, s.np, pend, ring, lane);
         if (rec) {  // the first document this range closes was parked by the helper: pick its value up again
             s.first = s.np;
             s.head = lds_f32(pend + (s.np * PEND_PITCH + lane) * 4);
@@ -1399,7 +1405,7 @@ dense_tc_kernel(const __grid_constant__ CUtensorMap map_docs, const Params p) {
             g += TSTEP;
             if (g >= NSEG) { g -= NSEG; gph ^= 1; }
         }
-        if (st.np) drain(pend, st.np, out, B, cfg, ring, lane);
+        if (st.np) drain(pend, st.np, out, B, cfg, lane);
     }
 
     // ---- teardown --------------------------------------------------------------------------------------------

@@ -300,3 +300,41 @@ def test_fuzz_shapes_against_the_oracle(seed):
     qi = synth.small_int_tokens(Q * Nq, d, dtype, seed=seed + 1).view(Q, Nq, d)
     Di = synth.small_int_tokens(int(off[-1]), d, dtype, seed=seed + 2)
     assert np.array_equal(run_dense(qi, Di, off, "tcgen05"), oracle.maxsim(qi, Di, off))
+
+
+# ---- parked documents outlive the ordinal ring (DOCRING wrap) ---------------------------------------------
+# A warp of two epilogue sets parks only the documents that end in ITS columns (column halves) or ITS tiles (alternate
+# tiles), up to 16 before it writes their scores, while the ordinal -> document ring (1024 entries) counts every document
+# of the CTA.  The periodic stores below make one set park a single document per tile (or per two tiles) while > 64
+# ordinals go by, so the 16 it holds span more than 1024 ordinals: the document index must have been resolved when the
+# document was parked, not when the buffer is drained.  Every CTA starts on a period boundary (the token count is a
+# multiple of 128 * SM count) and walks >= 24 tiles.
+
+def _periodic_offsets(block, periods):
+    return synth.offsets_from_lengths(np.tile(np.asarray(block, dtype=np.int64), periods))
+
+
+@pytest.mark.parametrize("Q", [4, 8])  # one and two query blocks per CTA
+def test_column_half_sets_with_one_long_and_64_single_token_documents_per_tile(Q):
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    off = _periodic_offsets([64] + [1] * 64, 24 * sms)
+    q, D = unit_case(Q, 32, 128, torch.bfloat16, off, seed=61)
+    assert_close(run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
+    # the mirrored tile: the set of the upper columns is the one that parks one document per tile
+    off = _periodic_offsets([1] * 64 + [64], 24 * sms)
+    q, D = unit_case(Q, 32, 128, torch.bfloat16, off, seed=63)
+    assert_close(run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
+
+
+def test_alternate_tile_sets_with_a_128_token_document_then_128_single_token_documents():
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    # the periodic part first (CTA 0 starts at token 0 and takes T / SMs tokens of it), then long documents that lift
+    # the mean length over 100 tokens, which is what selects the alternate-tile sets for one query block
+    periodic = np.tile(np.asarray([128] + [1] * 128, dtype=np.int64), 64)
+    n_long = 2 * sms
+    long_len = 128 * (-(-(100 * (periodic.size + n_long)) // (128 * n_long)))  # whole tiles: later CTAs stay aligned
+    lens = np.concatenate([periodic, np.full(n_long, long_len, dtype=np.int64)])
+    off = synth.offsets_from_lengths(lens)
+    assert off[-1] >= 100 * (off.size - 1) and off[-1] // sms >= 40 * 128
+    q, D = unit_case(4, 32, 64, torch.bfloat16, off, seed=65)
+    assert_close(run_dense(q, D, off, "tcgen05"), oracle.maxsim(q, D, off), tol(torch.bfloat16, 32))
