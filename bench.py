@@ -68,12 +68,12 @@ WORKLOADS = {
                       decode=True),
     "c5-decode-fp16": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16,
                            K=256, decode=True, precision="fp16"),
-    # configs[4] through tms_pq_maxsim as a caller gets it (TMS_VARIANT_AUTO: fp16 table entries in shared memory)
-    "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
-               pq_variant="pq_smem_f16"),
-    # the same LUT kernel over fp32 table entries (SURVEY 7.3 H6's A/B: twice the shared-memory gather bytes)
-    "c5-f32": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
-                   pq_variant="pq_smem"),
+    # configs[4] through tms_pq_maxsim as a caller gets it (TMS_VARIANT_AUTO: the paper's fp32 table, in shared
+    # memory); the kernel name and bytes per entry come from tms_pq_maxsim_variant_used, not from this table
+    "c5": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256),
+    # the opt-in LUT kernel over fp16 table entries (SURVEY 7.3 H6's A/B: half the shared-memory gather bytes, lossy)
+    "c5-f16": dict(kind="pq", Q=8, Nq=32, d=128, dtype="bf16", B=1_000_000, Nd=128, lengths="uniform", M=16, K=256,
+                   pq_variant="pq_smem_f16"),
 }
 TORCH_DTYPES = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32}
 ELEM_BYTES = {"bf16": 2, "fp16": 2, "fp32": 4}
@@ -129,6 +129,7 @@ class ClockSampler:
     def __init__(self, device_index: int, period_s: float = 0.005):
         self.period, self.samples, self.mask, self.h, self.max_mhz = period_s, [], 0, None, None
         self.power, self.power_limit = [], None
+        self.stamps, self.masks = [], []  # host time and throttle-reason mask of every sample
         self._stop = threading.Event()
         self._thread = None
         try:
@@ -153,9 +154,13 @@ class ClockSampler:
     def _run(self):
         while not self._stop.is_set():
             try:
-                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
-                self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
-                self.power.append(self._power_w())
+                mhz = int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                mask = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                pw = self._power_w()
+                self.stamps.append(time.perf_counter())
+                self.samples.append(mhz)
+                self.masks.append(mask)
+                self.power.append(pw)
             except Exception:
                 pass
             time.sleep(self.period)
@@ -178,10 +183,20 @@ class ClockSampler:
             self._thread = threading.Thread(target=self._run, daemon=True)
             self._thread.start()
 
-    def stop(self):
+    def stop(self, t_first=None, t_last=None):
+        """Ends sampling.  With [t_first, t_last] (host times between which the GPU was running the timed steps) only the
+        samples taken inside that window count: a sample read before the first step started shows the idle board."""
         if self._thread is not None:
             self._stop.set()
             self._thread.join()
+        if t_first is not None:
+            keep = [i for i, t in enumerate(self.stamps) if t_first <= t <= t_last]
+            self.samples = [self.samples[i] for i in keep]
+            self.power = [self.power[i] for i in keep]
+            self.masks = [self.masks[i] for i in keep]
+        self.mask = 0
+        for m in self.masks:
+            self.mask |= m
         reasons = [name for bit, name in self.REASONS.items() if self.mask & bit and name != "gpu_idle"]
         med = int(np.median(self.samples)) if self.samples else None
         out = {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": reasons, "samples": len(self.samples)}
@@ -351,14 +366,13 @@ class Workload:
             lut = torch.empty((Q, Nq, w["M"], w["K"]), dtype=torch.float32, device=dev)
             ws = torch.empty(max(tms.tms_pq_workspace_bytes(Q, Nq, w["M"], w["K"], B), 16), dtype=torch.uint8, device=dev)
 
-            # "c5" calls with variant "auto"; its `pq_variant` names what AUTO runs for that shape (roofline bytes per
-            # entry); "c5-f32" forces the fp32-entry kernel
-            pq_variant = variant if (variant != "auto" or name == "c5") else w.get("pq_variant", "auto")
+            # "c5" calls with variant "auto" and asks the library what that runs; "c5-f16" opts into fp16 entries
+            pq_variant = variant if variant != "auto" else w.get("pq_variant", "auto")
 
             def step():
                 tms.tms_pq_build_lut(inp["q"], inp["C"], lut=lut)
                 tms.tms_pq_maxsim(lut, inp["store"], self.off_d, scores=self.scores, workspace=ws, variant=pq_variant)
-            self.kernel = w.get("pq_variant", "pq_smem") if pq_variant == "auto" else pq_variant
+            self.kernel = tms.tms_pq_maxsim_variant_used(Q, Nq, w["M"], w["K"]) if pq_variant == "auto" else pq_variant
             self.entry_bytes = 2 if self.kernel == "pq_smem_f16" else 4
         self.step = step
 
@@ -368,18 +382,29 @@ def config_l2(w, T):
     return "inputs larger than L2 (no flush needed)" if big else "L2 flushed between timed steps"
 
 
-def timed_region(wl, steps, warmup, local_rank, sync_all, shard):
+def timed_region(wl, steps, warmup, local_rank, sync_all, shard, min_ms=0.0, max_steps=2000):
     """W warm-up steps, then exactly K steps with per-step CUDA events on the launching stream; clocks, throttle reasons and
-    board power are sampled through NVML while the steps run.  Returns per-step times and the max-over-ranks total."""
+    board power are sampled through NVML while the steps run (samples taken before the first step starts or after the
+    last one ends are dropped).  min_ms > 0 (secondary workloads): K is raised until the region lasts about min_ms, so
+    that the 5 ms NVML sampler sees it (at most max_steps).  Returns per-step times and the max-over-ranks total."""
+    w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0.record()
     for _ in range(warmup):
+        if wl.flush is not None:
+            wl.flush.fill_(1)
         wl.step()
+    w1.record()
     sync_all()
+    if min_ms > 0:
+        est = max(w0.elapsed_time(w1) / max(warmup, 1), 1e-3)  # ms per step, flush included
+        steps = int(min(max_steps, max(steps, np.ceil(min_ms / est))))
     sampler = ClockSampler(local_rank)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n0 = wl.tms.tms_launch_count()
     sampler.start()
     sync_all()
+    t_first = time.perf_counter() + 1e-3  # the GPU is idle here: the first step starts as soon as it is enqueued
     t_start.record()
     for a, b in ev:
         if wl.flush is not None:
@@ -388,8 +413,10 @@ def timed_region(wl, steps, warmup, local_rank, sync_all, shard):
         wl.step()
         b.record()
     t_end.record()
+    torch.cuda.synchronize()
+    t_last = time.perf_counter()
     sync_all()
-    clocks = sampler.stop()
+    clocks = sampler.stop(t_first, t_last)
     launches = wl.tms.tms_launch_count() - n0
     step_ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = float(step_ms.sum()) if wl.flush is not None else float(t_start.elapsed_time(t_end))
@@ -463,12 +490,15 @@ def roofline_of(wl, step_ms, total_ms, clocks, peaks):
 
 
 SECONDARY = ["c2-q4", "c2-q1", "c2-fp16", "c2-fp32", "c3-100k", "c3-250k", "c3-500k", "c4-d64", "c4-d256", "c4-d512",
-             "c4-d768", "c4-d512-q8", "c4-d768-q8", "c5", "c5-f32", "c5-decode", "c5-decode-fp16"]
+             "c4-d768", "c4-d512-q8", "c4-d768-q8", "c5", "c5-f16", "c5-decode", "c5-decode-fp16",
+             "c2-topk", "c1", "n1-b1k", "n1-nq64", "n1-nd32", "n1-nd512"]
+SECONDARY_MIN_MS = 150.0  # each secondary timed region lasts at least this long (>= 20 NVML samples under load)
 
 
 def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):
-    """The other BASELINE.json configs, each timed briefly (its own warm-up, 5 steps, its own clock samples) AFTER and
-    outside the headline's timed region: {name: {ms_per_step, docs_per_s, bound, frac, ...}}."""
+    """The other BASELINE.json configs and the NEXT-1 sweeps' end points, each timed on its own (its own warm-up, at least
+    --secondary-steps steps and at least SECONDARY_MIN_MS of device time, its own clock samples taken under load) AFTER
+    and outside the headline's timed region: {name: {ms_per_step, docs_per_s, bound, frac, ...}}."""
     out = {}
     prev = main_wl
     for name in SECONDARY:
@@ -476,19 +506,24 @@ def run_secondary(args, main_wl, dev, local_rank, tms, shard, sync_all, peaks):
             continue
         w = WORKLOADS[name]
         try:
-            wl = Workload(name, w, w["B"], args.seed, dev, tms, reuse=prev)
+            same_store = [c for c in (prev, main_wl) if c.w["kind"] == w["kind"] == "dense" and c.B == w["B"] and
+                          all(c.w[k] == w[k] for k in ("d", "dtype", "lengths", "Nd"))]
+            wl = Workload(name, w, w["B"], args.seed, dev, tms, reuse=same_store[0] if same_store else None)
             torch.cuda.synchronize()
             time.sleep(1.0)  # let the board's power controller settle after the previous workload (each config is timed
             #                  on its own: a 0.4 ms kernel measured right behind a power-capped one inherits its clocks)
-            step_ms, total_ms, clocks, launches = timed_region(wl, args.secondary_steps, 3, local_rank, sync_all, shard)
+            step_ms, total_ms, clocks, launches = timed_region(wl, args.secondary_steps, 3, local_rank, sync_all, shard,
+                                                               min_ms=SECONDARY_MIN_MS)
             r = roofline_of(wl, step_ms, total_ms, clocks, peaks)
             out[name] = {"ms_per_step": float(step_ms.mean()), "ms_min": float(step_ms.min()),
-                         "docs_per_s": w["B"] / (float(step_ms.mean()) * 1e-3), "steps": args.secondary_steps,
+                         "ms_median": float(np.median(step_ms)),
+                         "docs_per_s": w["B"] / (float(step_ms.mean()) * 1e-3), "steps": int(step_ms.size),
                          "bound": r["bound"], "frac": r["frac"], "achieved": r["achieved"], "peak": r["peak"],
                          "unit": r["unit"], "hbm_GBps": r["hbm"]["achieved_GBps"], "hbm_frac": r["hbm"]["frac"],
                          "tensor_frac_burst": r.get("tensor", {}).get("frac_burst"), "kernel": r["kernel"],
                          "gpu_launches": launches, "traffic": r["traffic"],
-                         "clocks": {k: clocks.get(k) for k in ("sm_mhz", "reasons", "power_w_mean", "power_w_max")},
+                         "clocks": {k: clocks.get(k) for k in ("sm_mhz", "reasons", "samples", "power_w_mean",
+                                                               "power_w_max")},
                          "B": w["B"], "total_tokens": wl.T}
             if prev is not main_wl and prev is not wl:
                 del prev
@@ -511,8 +546,23 @@ def spawn_ranks(args):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
-    raise SystemExit(subprocess.call(cmd, env=env))
+    env.setdefault("NCCL_DEBUG", "INFO")        # communicator / transport lines (NVLS, P2P) for whoever checks the ranks
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    # NCCL writes to stdout, from every rank and also at teardown: pass everything through as it comes, but hold rank 0's
+    # JSON line back so that it is the LAST line of this process's stdout
+    proc = subprocess.Popen(cmd, env=env, stdout=subprocess.PIPE, text=True, bufsize=1)
+    final = None
+    for ln in proc.stdout:
+        if ln.startswith("{") and '"metric"' in ln:
+            final = ln
+        else:
+            sys.stdout.write(ln)
+            sys.stdout.flush()
+    rc = proc.wait()
+    if final is not None:
+        sys.stdout.write(final)
+        sys.stdout.flush()
+    raise SystemExit(rc)
 
 
 def main():
@@ -528,7 +578,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the brief timings of the other configs")
-    ap.add_argument("--secondary-steps", type=int, default=5)
+    ap.add_argument("--secondary-steps", type=int, default=20)
+    ap.add_argument("--sustained-steps", type=int, default=200,
+                    help="steps of the headline's separate long run (0 = skip)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "tms" else args.warmup
@@ -597,6 +649,26 @@ def main():
     # ---- the other configs, briefly, outside the headline's timed region (single-GPU runs only) ----------------------
     if world == 1 and not args.no_secondary and args.workload == "c2" and not args.B:
         line["secondary"] = run_secondary(args, wl, dev, local_rank, tms, shard, sync_all, peaks)
+    # ---- the headline again as one long run ("sustains", north_star): outside the K-step region, after a pause ---------
+    line["step_ms"] = [round(float(x), 4) for x in step_ms]
+    if args.sustained_steps > 0:
+        torch.cuda.synchronize()
+        time.sleep(1.0)
+        s_ms, s_total, s_clk, _ = timed_region(wl, args.sustained_steps, 3, local_rank, sync_all, shard)
+        rs = roofline_of(wl, s_ms, s_total, s_clk, peaks)
+        line["sustained"] = {"steps": int(s_ms.size), "ms_per_step": s_total / s_ms.size,
+                             "ms_median": float(np.median(s_ms)), "bound": rs["bound"], "frac_burst": rs["frac"],
+                             "frac_sustained": rs.get("tensor", {}).get("frac_sustained") if rs["bound"] == "tensor"
+                             else None, "hbm_frac": rs["hbm"]["frac"],
+                             "sm_mhz": s_clk.get("sm_mhz"), "reasons": s_clk.get("reasons"),
+                             "samples": s_clk.get("samples"), "power_w_mean": s_clk.get("power_w_mean")}
+    # compact copy of every secondary result, LAST in the line so that a truncated record still carries all of them:
+    # name -> [ms mean, ms median, bound, fraction of that bound's peak, steps, NVML samples under load, median SM MHz]
+    if "secondary" in line:
+        line["secondary_summary"] = {
+            n: ([round(v["ms_per_step"], 5), round(v["ms_median"], 5), v["bound"], round(v["frac"], 4), v["steps"],
+                 v["clocks"].get("samples"), v["clocks"].get("sm_mhz")] if "error" not in v else ["error"])
+            for n, v in line["secondary"].items()}
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

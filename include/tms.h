@@ -59,9 +59,9 @@ typedef enum {
     TMS_VARIANT_AUTO = 0,     /* what tms_maxsim / tms_pq_maxsim pick                                  */
     TMS_VARIANT_SIMT = 1,     /* CUDA-core tiled kernel: any dtype, any d, any Nq (the general path)   */
     TMS_VARIANT_TCGEN05 = 2,  /* TMA + tcgen05 tensor-core kernel (sm_100a), dimension-tiled for d>128 */
-    TMS_VARIANT_PQ_SMEM = 3,  /* PQ: LUT slices resident in shared memory                              */
-    TMS_VARIANT_PQ_SMEM_F16 = 4 /* PQ: the same with table entries held as (block-scaled) fp16 in shared memory:
-                                 half the gather bytes; see tms_pq_maxsim                                */
+    TMS_VARIANT_PQ_SMEM = 3,  /* PQ: LUT slices resident in shared memory, fp32 entries (AUTO's choice)    */
+    TMS_VARIANT_PQ_SMEM_F16 = 4 /* PQ, opt-in only: the same with table entries held as (block-scaled) fp16 in
+                                 shared memory: half the gather bytes, lossy; see tms_pq_maxsim          */
 } tms_variant;
 
 /*
@@ -89,8 +89,9 @@ typedef enum {
  * (Eq. 7).
  * d > 128 accumulates partial dot products over dimension chunks before the max is taken.
  * Stores of 2^31 - 128 tokens or more (TMA tile coordinates are 32-bit) are scored in segments of 2^30 tokens, one
- * launch per segment; a single document must then be shorter than 2^30 tokens.  The same holds for
- * tms_pq_maxsim_decode.
+ * launch per segment; a single document must then be no longer than 2^30 - 128 tokens (it may start on a segment's
+ * last token and must end inside the next segment's tensor map; a longer one is scored wrongly, without an error --
+ * lengths live in device memory).  The same holds for tms_pq_maxsim_decode.
  */
 int tms_maxsim(const void* queries, int Q, int Nq, int d, const void* docs, const int64_t* offsets, int64_t B,
                int64_t total_tokens, tms_dtype dtype, float* scores, void* workspace, size_t workspace_bytes,
@@ -127,14 +128,22 @@ int tms_pq_build_lut(const void* queries, int Q, int Nq, int d, tms_dtype q_dtyp
  * The decompressed vectors are never materialised.  The sum over m is fp32 in a fixed, kernel-defined
  * order (run-to-run reproducible).
  * workspace  device scratch of at least tms_pq_workspace_bytes(...) bytes (the re-laid-out table).
- * Kernels: for M = 16, K = 256 the table is re-laid-out into the workspace and served from shared memory in slices
- * (P:L268 keeps it in L2; here the gathers are the bound).  With Nq % 16 == 0 the re-laid-out copy holds the entries
- * as fp16 after one power-of-two scale of the whole table (max|entry| -> [2^14, 2^15): no overflow or subnormals for
- * any finite table), they are widened back inside the fp32 additions, and the scale is undone exactly: half the
- * gather bytes, one rounding of relative 2^-11 per entry (measured max |dscore| on config 4's data: see DESIGN.md
- * 5.4; tests hold it to a quarter of the 2e-3*Nq tolerance).  TMS_VARIANT_PQ_SMEM forces fp32 entries (Nq % 8 == 0),
- * TMS_VARIANT_PQ_SMEM_F16 the fp16 ones, TMS_VARIANT_SIMT the general kernel (any M, K <= 256, Nq; table read
- * through L1/L2).  `lut` itself is never modified.
+ * Precision contract: tms_pq_maxsim (TMS_VARIANT_AUTO) adds the fp32 table entries as they are (the paper's table is
+ * fp32) -- the only rounding is the fp32 sum over m and, before it, the fp32 FMA chain of tms_pq_build_lut.
+ * Whatever the queries' dtype was, the scores are within 1e-5 * Nq * max|dhat| of Eq. 9 evaluated on the stored query
+ * values (so within the 1e-5*Nq bound of fp32 inputs and, a fortiori, the 2e-3*Nq bound of 16-bit ones).  The call
+ * cannot know what `lut` was built from and therefore never narrows it on its own.
+ * Kernels: for M = 16, K = 256, Nq % 8 == 0 the table is re-laid-out into the workspace and served from shared memory
+ * in 8-row slices (P:L268 keeps it in L2; here the gathers are the bound): TMS_VARIANT_PQ_SMEM, what AUTO picks for
+ * that shape; any other shape (any M, K <= 256, Nq) runs the general kernel, TMS_VARIANT_SIMT, with the table read
+ * through L1/L2.
+ * OPT-IN, through tms_pq_maxsim_variant only: TMS_VARIANT_PQ_SMEM_F16 (Nq % 16 == 0) holds the re-laid-out copy as fp16
+ * after one power-of-two scale of the whole table (max|entry| -> [2^14, 2^15): no overflow or subnormals for any
+ * finite table); entries are widened back inside the fp32 additions and the scale is undone exactly.  Half the gather
+ * bytes (1.9x faster on config 5) for one rounding of relative 2^-11 per entry: |dscore| <= Nq * M * max|entry| * 2^-12
+ * in the worst case, ~2e-3 measured on config 5's data -- inside the 2e-3*Nq tolerance of 16-bit
+ * queries, NOT inside the 1e-5*Nq one of fp32 queries, and near-ties in a ranking can swap.  Choose it only for tables
+ * built from 16-bit queries.  `lut` itself is never modified.
  */
 int tms_pq_maxsim(const float* lut, int Q, int Nq, int M, int K, const uint8_t* codes, const int64_t* offsets,
                   int64_t B, int64_t total_tokens, float* scores, void* workspace, size_t workspace_bytes,
@@ -145,6 +154,11 @@ int tms_pq_maxsim_variant(const float* lut, int Q, int Nq, int M, int K, const u
                           size_t workspace_bytes, void* stream, tms_variant variant);
 
 size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B);
+
+/* Which kernel tms_pq_maxsim (TMS_VARIANT_AUTO) runs for this shape: TMS_VARIANT_PQ_SMEM (fp32 entries in shared
+ * memory) or TMS_VARIANT_SIMT (the general kernel); never TMS_VARIANT_PQ_SMEM_F16.  TMS_VARIANT_AUTO for non-positive
+ * sizes.  A pure function of its arguments: no device is touched. */
+int tms_pq_maxsim_variant_used(int Q, int Nq, int M, int K);
 
 /*
  * Decode-and-contract PQ scoring: the same value as tms_pq_build_lut + tms_pq_maxsim,
@@ -271,7 +285,9 @@ size_t tms_topk_static_scratch_bytes(void);
  *         (values[g, q, r], shard_base[g] + indices[g, q, r]),  same order as tms_topk (score descending, lower GLOBAL
  *         document index first, -INFINITY last).  With k_in >= k this equals tms_topk over the concatenated scores.
  * values / indices   device, fp32 / int64 [G, Q, k_in] (shard-local document indices, as tms_topk wrote them).
- * shard_base         HOST, int64 [G]: first global document index of every shard; 0 <= base, base + index < 2^31.
+ * shard_base         HOST, int64 [G]: first global document index of every shard; 0 <= base < 2^31 (else
+ *                    TMS_ERR_INVALID_ARG).  base + index < 2^31 for every candidate is the caller's contract: the
+ *                    indices live in device memory, the host cannot check them, and a larger sum wraps silently.
  * G <= 64; k, k_in <= 1024; k <= G*k_in.  workspace: device, >= tms_topk_merge_workspace_bytes(...), 8-byte aligned.
  */
 int tms_topk_merge(const float* values, const int64_t* indices, const int64_t* shard_base, int G, int Q, int k_in, int k,

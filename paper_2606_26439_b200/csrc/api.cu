@@ -115,11 +115,12 @@ static int pq_dispatch(const float* lut, int Q, int Nq, int M, int K, const uint
     if (variant != TMS_VARIANT_AUTO && variant != TMS_VARIANT_SIMT && variant != TMS_VARIANT_PQ_SMEM &&
         variant != TMS_VARIANT_PQ_SMEM_F16)
         return TMS_ERR_INVALID_ARG;
-    // AUTO: the shared-memory kernel over fp16 table entries when the shape has whole 16-row slices (half the gather
-    // bytes, 1.9x faster on config 4, error well inside the 16-bit tolerance: DESIGN.md 5.4), else over fp32 entries
-    // (8-row slices), else the general kernel.  TMS_VARIANT_PQ_SMEM always means fp32 entries.
+    // AUTO never narrows the table: the call sees only `lut`, not what it was built from, and a table built from fp32
+    // queries is held to 1e-5*Nq (the paper's table is fp32).  AUTO = the shared-memory kernel over fp32 entries
+    // when the shape has whole 8-row slices, else the general kernel.  fp16 entries (half the gather bytes, 1.9x faster
+    // on config 5, one 2^-11 rounding per entry: DESIGN.md 5.4) are the caller's explicit choice: TMS_VARIANT_PQ_SMEM_F16.
     PqArgs a{lut, Q, Nq, M, K, codes, offsets, B, T, scores, static_cast<cudaStream_t>(stream)};
-    const bool f16 = variant == TMS_VARIANT_PQ_SMEM_F16 || (variant == TMS_VARIANT_AUTO && pq_smem_supports(a, true));
+    const bool f16 = variant == TMS_VARIANT_PQ_SMEM_F16;
     const bool smem_ok = pq_smem_supports(a, f16);
     if (variant == TMS_VARIANT_SIMT || (variant == TMS_VARIANT_AUTO && !smem_ok)) return launch_pq_simt(a);
     if (!smem_ok) return TMS_ERR_UNSUPPORTED;
@@ -186,6 +187,12 @@ int tms_pq_maxsim_variant(const float* lut, int Q, int Nq, int M, int K, const u
                           size_t workspace_bytes, void* stream, tms_variant variant) {
     return pq_dispatch(lut, Q, Nq, M, K, codes, offsets, B, total_tokens, scores, workspace, workspace_bytes, stream,
                        variant);
+}
+
+int tms_pq_maxsim_variant_used(int Q, int Nq, int M, int K) {
+    if (Q <= 0 || Nq <= 0 || M <= 0 || K <= 0) return TMS_VARIANT_AUTO;  // nothing is scored
+    PqArgs a{nullptr, Q, Nq, M, K, nullptr, nullptr, 0, 0, nullptr, nullptr};
+    return pq_smem_supports(a, false) ? TMS_VARIANT_PQ_SMEM : TMS_VARIANT_SIMT;
 }
 
 size_t tms_pq_workspace_bytes(int Q, int Nq, int M, int K, int64_t B) {
@@ -273,7 +280,7 @@ int tms_topk_merge(const float* values, const int64_t* indices, const int64_t* s
     if ((int64_t)k > (int64_t)G * k_in) return TMS_ERR_INVALID_ARG;
     if (G > 64 || k > 1024 || k_in > 1024 || Q > 65535) return TMS_ERR_UNSUPPORTED;
     for (int g = 0; g < G; ++g)
-        if (shard_base[g] < 0 || shard_base[g] > (1ll << 31)) return TMS_ERR_INVALID_ARG;
+        if (shard_base[g] < 0 || shard_base[g] >= (1ll << 31)) return TMS_ERR_INVALID_ARG;  // base + index < 2^31
     if ((reinterpret_cast<uintptr_t>(values) & 3u) || (reinterpret_cast<uintptr_t>(out_values) & 3u) ||
         (reinterpret_cast<uintptr_t>(indices) & 7u) || (reinterpret_cast<uintptr_t>(out_indices) & 7u))
         return TMS_ERR_ALIGNMENT;

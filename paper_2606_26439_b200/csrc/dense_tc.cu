@@ -1711,8 +1711,9 @@ int launch_dense_tc(const DenseArgs& a) {
     if (!ensure_smem_attr(reinterpret_cast<const void*>(kern), di->device, pl.smem_bytes)) return TMS_ERR_CUDA;
     // TMA tile coordinates are 32-bit: a store of 2^31 - 128 tokens or more is scored in token segments of 2^30 tokens,
     // one launch per segment (and query group), each with a tensor map that starts at the segment's first token.  A
-    // document belongs to the segment its first token lies in and may reach into the next one (documents are shorter
-    // than 2^30 tokens by contract).  Smaller stores are one segment.
+    // document belongs to the segment its first token lies in and may reach into the next one (by contract no document
+    // of such a store is longer than 2^30 - 128 tokens: one that starts on a segment's last token then still ends
+    // inside map_rows below).  Smaller stores are one segment.
     const int64_t SEG = 1ll << 30;
     const int64_t nseg = a.T < (1ll << 31) - BN ? 1 : (a.T + SEG - 1) / SEG;
     // one launch per group of Qg queries (up to 256 query rows): the store is streamed once per group

@@ -31,6 +31,7 @@ SIGNATURES = {
     "tms_pq_maxsim": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
     "tms_pq_workspace_bytes": (_sz, [_i, _i, _i, _i, _i64]),
+    "tms_pq_maxsim_variant_used": (_i, [_i, _i, _i, _i]),
     "tms_pq_maxsim_decode": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp]),
     "tms_pq_maxsim_decode_variant": (_i, [_vp, _i, _i, _i, _i, _vp, _i, _i, _vp, _vp, _i64, _i64, _vp, _vp, _sz, _vp, _i]),
     "tms_maxsim_host": (_i, [_vp, _i, _i, _i, _vp, _vp, _i64, _i64, _i, _vp, _vp, _sz, _vp]),
@@ -100,6 +101,12 @@ def tms_maxsim_workspace_bytes(Q, Nq, d, B, dtype) -> int:
 def tms_maxsim_variant_used(Q, Nq, d, B, total_tokens, dtype) -> str:
     """Name of the kernel tms_maxsim picks for this shape ("tcgen05" / "simt"; "auto" when nothing is scored)."""
     v = int(load().tms_maxsim_variant_used(Q, Nq, d, B, total_tokens, _DTYPES[dtype]))
+    return {val: name for name, val in VARIANTS.items()}[v]
+
+
+def tms_pq_maxsim_variant_used(Q, Nq, M, K) -> str:
+    """Name of the kernel tms_pq_maxsim picks for this shape ("pq_smem" = fp32 entries in shared memory, or "simt")."""
+    v = int(load().tms_pq_maxsim_variant_used(Q, Nq, M, K))
     return {val: name for name, val in VARIANTS.items()}[v]
 
 

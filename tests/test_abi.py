@@ -42,7 +42,7 @@ def test_binding_covers_every_declared_symbol():
 def test_status_strings_and_version(lib):
     assert lib.tms_version() >= 100
     assert lib.tms_status_string(0) == b"ok"
-    assert len({lib.tms_status_string(i) for i in range(6)}) == 6
+    assert len({lib.tms_status_string(i) for i in range(7)}) == 7
 
 
 def test_workspace_size_functions(lib):
@@ -50,6 +50,31 @@ def test_workspace_size_functions(lib):
     assert lib.tms_pq_workspace_bytes(8, 32, 16, 256, 1000000) == 8 * 32 * 16 * 256 * 4 + 16  # table + header
     assert lib.tms_pq_workspace_bytes(8, 32, 8, 256, 1000) == 0
     assert lib.tms_maxsim_host_workspace_min_bytes(8, 32, 128, tms.TMS_DTYPE_BF16, 180) > 2 * 180 * 256
+
+
+def test_pq_variant_used_is_a_pure_function_and_never_the_lossy_kernel(lib):
+    assert lib.tms_pq_maxsim_variant_used(8, 32, 16, 256) == tms.TMS_VARIANT_PQ_SMEM   # configs[4]: fp32 entries
+    assert lib.tms_pq_maxsim_variant_used(8, 24, 16, 256) == tms.TMS_VARIANT_PQ_SMEM
+    assert lib.tms_pq_maxsim_variant_used(5, 7, 16, 256) == tms.TMS_VARIANT_SIMT
+    assert lib.tms_pq_maxsim_variant_used(2, 12, 8, 64) == tms.TMS_VARIANT_SIMT
+    assert lib.tms_pq_maxsim_variant_used(0, 32, 16, 256) == tms.TMS_VARIANT_AUTO
+    assert tms.tms_pq_maxsim_variant_used(8, 32, 16, 256) == "pq_smem"
+
+
+def test_topk_merge_rejects_a_shard_base_of_2_to_the_31(lib):
+    buf = (ctypes.c_char * 4096)()
+    p16 = (ctypes.addressof(buf) + 15) & ~15
+    for bad in (1 << 31, -1):
+        base = (ctypes.c_int64 * 2)(0, bad)
+        assert lib.tms_topk_merge(p16, p16, ctypes.addressof(base), 2, 1, 4, 4, p16, p16, p16, 4096, None) == 1
+
+
+def test_static_topk_limit_is_reported_without_a_device(lib):
+    assert lib.tms_topk_static_scratch_bytes() == 4 << 20
+    buf = (ctypes.c_char * 4096)()
+    p16 = (ctypes.addressof(buf) + 15) & ~15
+    assert lib.tms_topk_static(p16, 8, 1_000_000, 1024, p16, p16, None) == 6  # refused before any CUDA call
+    assert b"static buffer" in lib.tms_status_string(6)
 
 
 def test_argument_validation_happens_before_any_cuda_call(lib):

@@ -15,6 +15,7 @@ import pytest
 import torch
 
 import oracle
+import planting
 from paper_2606_26439_b200 import synth, tms
 
 pytestmark = pytest.mark.gpu
@@ -48,7 +49,7 @@ def dense_fullsize(Q, Nq, d, dtype, off, seed, n_sample=1500, planted=True):
     B, T = len(off) - 1, int(off[-1])
     q = synth.unit_tokens(Q * Nq, d, dtype, seed=seed + 1, device=DEV).view(Q, Nq, d)
     D = synth.unit_tokens(T, d, dtype, seed=seed + 2, device=DEV)
-    ids_planted = synth.plant_relevant(q, D, off, seed=seed + 3) if planted else np.zeros((Q, 0), np.int64)
+    ids_planted = planting.plant_relevant(q, D, off, seed=seed + 3) if planted else np.zeros((Q, 0), np.int64)
     off_d = torch.from_numpy(off).to(DEV)
     got_d = tms.tms_maxsim(q, D, off_d)          # the call bench.py makes (variant "auto")
     again = tms.tms_maxsim(q, D, off_d)
@@ -111,7 +112,7 @@ def test_config4_fused_pq():
     q = synth.unit_tokens(Q * Nq, d, torch.bfloat16, seed=401, device=DEV).view(Q, Nq, d)
     C = synth.pq_codebooks(M, K, d // M, seed=402)
     codes = synth.pq_codes(int(off[-1]), M, seed=403, device=DEV, K=K)
-    ids_planted = synth.plant_relevant_pq(q, C, codes, off, seed=405)   # 32 planted documents per query, in rank order
+    ids_planted = planting.plant_relevant_pq(q, C, codes, off, seed=405)   # 32 planted documents per query, in rank order
     off_d = torch.from_numpy(off).to(DEV)
     lut = tms.tms_pq_build_lut(q, C.to(DEV))
     got_d = tms.tms_pq_maxsim(lut, codes, off_d)
@@ -144,15 +145,20 @@ def test_config4_fused_pq():
     dec = dec_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
     assert np.abs(dec - ref).max() <= 2e-3 * Nq
     ranking_rule(dec, ref, 2e-3 * Nq)
-    # all 8,000,000 scores of three independent kernels agree: the decode variant, the LUT kernel over fp32 table entries,
-    # and what tms_pq_maxsim runs by default for this shape (fp16 table entries, a quarter of the tolerance at most)
+    # all 8,000,000 scores of three independent kernels agree: the decode variant, the LUT kernel over fp32 table entries
+    # (what tms_pq_maxsim runs by default for this shape: bit-identical to naming it), and the opt-in LUT kernel over
+    # fp16 table entries (a quarter of the 16-bit tolerance at most)
+    assert tms.tms_pq_maxsim_variant_used(Q, Nq, M, K) == "pq_smem"
     f32_d = tms.tms_pq_maxsim(lut, codes, off_d, variant="pq_smem")
+    assert torch.equal(got_d, f32_d)
     assert float((dec_d - f32_d).abs().max()) < 5e-4
-    for other in (dec_d, f32_d):
+    f16_d = tms.tms_pq_maxsim(lut, codes, off_d, variant="pq_smem_f16")
+    for other in (dec_d, f16_d):
         assert np.array_equal(torch.topk(other, KTOP, dim=1).indices.cpu().numpy(), ids_planted[:, :KTOP])
-    assert float((got_d - f32_d).abs().max()) <= 0.25 * 2e-3 * Nq
-    f32 = f32_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
-    assert np.abs(f32 - ref).max() <= 2e-3 * Nq
+    assert float((f16_d - f32_d).abs().max()) <= 0.25 * 2e-3 * Nq
+    f16 = f16_d[:, torch.from_numpy(sample).to(DEV)].cpu().numpy().astype(np.float64)
+    assert np.abs(f16 - ref).max() <= 2e-3 * Nq
+    ranking_rule(f16, ref, 2e-3 * Nq)
 
 
 # ---- stores of 2^31 tokens and more: TMA coordinates are 32-bit, the library scores them in 2^30-token segments ---------

@@ -105,6 +105,33 @@ def test_f16_table_is_block_scaled(scale):
     assert_close(h / scale, ref / scale, 0.25 * 2e-3 * 16)
 
 
+@pytest.mark.parametrize("q_dtype", [torch.float32, torch.bfloat16, torch.float16])
+@pytest.mark.parametrize("Nq", [32, 48, 20])  # 16-row slices possible / 8-row slices only / the general kernel
+def test_auto_keeps_the_fp32_table_whatever_it_was_built_from(q_dtype, Nq):
+    """tms_pq_maxsim sees only `lut`, not the queries' dtype, so its default must hold the tightest bound an input class
+    carries: 1e-5*Nq for fp32 queries (north_star; scaled by max|dhat| as in test_p13), 2e-3*Nq for 16-bit ones.  The
+    paper's table is fp32; fp16 entries are opt-in and are NOT inside the fp32 bound on this data."""
+    lens = np.concatenate([[5, 128, 1, 0, 300, 16, 17, 15, 0, 0, 33, 1000],
+                           synth.lognormal_lengths(3000, seed=31, median=60, lo=0, hi=200)])
+    off = synth.offsets_from_lengths(lens)
+    q, C, codes = pq_case(8, Nq, 16, 256, 8, off, seed=33, q_dtype=q_dtype)
+    ref = oracle.pq_maxsim(q, C, codes, off)
+    dhat_norm = float(np.sqrt((C.double().numpy() ** 2).sum(-1).max(-1).sum()))  # max over codes of ||dhat||
+    _, auto = run_pq(q, C, codes, off)  # TMS_VARIANT_AUTO
+    want = "pq_smem" if Nq % 8 == 0 else "simt"
+    assert tms.tms_pq_maxsim_variant_used(8, Nq, 16, 256) == want
+    _, named = run_pq(q, C, codes, off, want)
+    assert np.array_equal(auto, named)
+    assert_close(auto, ref, 1e-5 * Nq * max(1.0, dhat_norm))   # the fp32 bound holds for EVERY query dtype
+    tol_16 = 2e-3 * Nq
+    assert_close(auto, ref, tol_16)
+    if Nq % 16 == 0:  # the opt-in: inside the 16-bit bound, outside the fp32 one (which is why it is not the default)
+        _, h = run_pq(q, C, codes, off, "pq_smem_f16")
+        assert_close(h, ref, tol_16)
+        fin = np.isfinite(ref)
+        assert np.abs(h[fin] - ref[fin]).max() > 1e-5 * Nq * max(1.0, dhat_norm)
+
+
 def test_f16_table_needs_whole_16_row_slices():
     off = synth.uniform_offsets(50, 20)
     q, C, codes = pq_case(2, 24, 16, 256, 8, off, seed=25)   # Nq = 24: fine for the fp32 table (8-row slices) only
@@ -157,8 +184,10 @@ def test_decode_variant_matches_the_oracle_and_the_lut_path(q_dtype, Q):
     assert np.abs(got[fin] - ref[fin]).max() < 2e-4  # hi/lo split: far inside the tolerance
     _, lut_scores = run_pq(q, C, codes, off, "pq_smem")       # the LUT kernel over fp32 table entries
     assert np.abs(got[fin] - lut_scores[fin]).max() < 2e-4
-    _, auto_scores = run_pq(q, C, codes, off)                 # what tms_pq_maxsim runs by default: fp16 table entries
-    assert np.abs(got[fin] - auto_scores[fin]).max() <= 0.25 * 2e-3 * 32
+    _, auto_scores = run_pq(q, C, codes, off)                 # what tms_pq_maxsim runs by default: the same fp32 entries
+    assert np.array_equal(auto_scores, lut_scores)
+    _, f16_scores = run_pq(q, C, codes, off, "pq_smem_f16")   # the opt-in fp16 entries
+    assert np.abs(got[fin] - f16_scores[fin]).max() <= 0.25 * 2e-3 * 32
 
 
 def test_decode_variant_exact_on_integer_codebooks():

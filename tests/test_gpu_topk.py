@@ -5,6 +5,7 @@ import pytest
 import torch
 
 import oracle
+import planting
 from paper_2606_26439_b200 import synth, tms
 
 pytestmark = pytest.mark.gpu
@@ -40,7 +41,7 @@ def test_topk_of_real_scores_equals_topk_of_oracle_scores_on_planted_documents()
     off = synth.uniform_offsets(B, 64)
     q = synth.unit_tokens(Q * Nq, d, torch.bfloat16, seed=1).view(Q, Nq, d)
     D = synth.unit_tokens(int(off[-1]), d, torch.bfloat16, seed=2)
-    ids = synth.plant_relevant(q, D, off, seed=3)
+    ids = planting.plant_relevant(q, D, off, seed=3)
     scores = tms.tms_maxsim(q.to(DEV), D.to(DEV), torch.from_numpy(off).to(DEV))
     vals, idx = tms.tms_topk(scores, 100)
     assert np.array_equal(idx.cpu().numpy(), ids[:, :100])  # planted documents, in order (gaps twice the tolerance)

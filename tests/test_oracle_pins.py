@@ -12,6 +12,7 @@ import pytest
 import torch
 
 import oracle
+import planting
 from paper_2606_26439_b200 import synth
 
 DTYPES = [torch.float32, torch.float16, torch.bfloat16]
@@ -279,7 +280,7 @@ def test_planted_documents_rank_first_in_order():
     q = synth.unit_tokens(Q * Nq, d, torch.bfloat16, seed=1).view(Q, Nq, d)
     D = synth.unit_tokens(B * Nd, d, torch.bfloat16, seed=2)
     off = synth.uniform_offsets(B, Nd)
-    ids = synth.plant_relevant(q, D, off, seed=3, per_query=50)
+    ids = planting.plant_relevant(q, D, off, seed=3, per_query=50)
     s = oracle.maxsim(q, D, off)
     for qq in range(Q):
         top = np.argsort(-s[qq], kind="stable")[:50]

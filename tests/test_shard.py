@@ -134,16 +134,29 @@ def test_bench_gpus_flag_spawns_its_own_ranks():
     spec.loader.exec_module(bench)
     seen = {}
 
-    def fake_call(cmd, env=None):
-        seen["cmd"], seen["env"] = cmd, env
-        return 0
+    class FakeRanks:  # stands in for the torchrun child: NCCL chatter before AND after rank 0's JSON line
+        def __init__(self, cmd, env=None, **kw):
+            seen["cmd"], seen["env"] = cmd, env
+            self.stdout = iter(["rank 1 NCCL INFO Init START\n", '{"metric": "m", "value": 1}\n',
+                                "rank 3 NCCL INFO comm destroyed\n"])
+
+        def wait(self):
+            return 0
 
     argv = ["bench.py", "--gpus", "4", "--steps", "2", "--warmup", "3"]
-    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
-    with mock.patch.object(sys, "argv", argv), mock.patch("subprocess.call", fake_call), \
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "NCCL_DEBUG")}
+    import io
+    out = io.StringIO()
+    with mock.patch.object(sys, "argv", argv), mock.patch("subprocess.Popen", FakeRanks), \
+            mock.patch.object(sys, "stdout", out), \
             mock.patch.dict(os.environ, env, clear=True), pytest.raises(SystemExit) as e:
         bench.main()
     assert e.value.code == 0
     cmd = seen["cmd"]
     assert "torch.distributed.run" in cmd and "--nproc-per-node=4" in cmd and "127.0.0.1" in cmd
-    assert cmd[-6:] == argv[1:] and "NCCL_DEBUG" in seen["env"]
+    assert cmd[-6:] == argv[1:]
+    # communicator lines are on by default (the driver's rank check reads them) ...
+    assert seen["env"]["NCCL_DEBUG"] == "INFO" and seen["env"]["NCCL_DEBUG_SUBSYS"] == "INIT"
+    # ... and rank 0's JSON line is still the LAST line of stdout
+    lines = out.getvalue().splitlines()
+    assert len(lines) == 3 and lines[-1].startswith('{"metric"') and "comm destroyed" in lines[1]
