@@ -387,16 +387,19 @@ def timed_region(wl, steps, warmup, local_rank, sync_all, shard, min_ms=0.0, max
     board power are sampled through NVML while the steps run (samples taken before the first step starts or after the
     last one ends are dropped).  min_ms > 0 (secondary workloads): K is raised until the region lasts about min_ms, so
     that the 5 ms NVML sampler sees it (at most max_steps).  Returns per-step times and the max-over-ranks total."""
-    w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    w0.record()
     for _ in range(warmup):
-        if wl.flush is not None:
-            wl.flush.fill_(1)
         wl.step()
-    w1.record()
     sync_all()
-    if min_ms > 0:
-        est = max(w0.elapsed_time(w1) / max(warmup, 1), 1e-3)  # ms per step, flush included
+    if min_ms > 0:  # a few more untimed steps, measured, to size the region (flush included; first-call costs excluded)
+        w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        w0.record()
+        for _ in range(5):
+            if wl.flush is not None:
+                wl.flush.fill_(1)
+            wl.step()
+        w1.record()
+        sync_all()
+        est = max(w0.elapsed_time(w1) / 5, 1e-3)
         steps = int(min(max_steps, max(steps, np.ceil(min_ms / est))))
     sampler = ClockSampler(local_rank)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]

@@ -129,7 +129,7 @@ def test_auto_keeps_the_fp32_table_whatever_it_was_built_from(q_dtype, Nq):
         _, h = run_pq(q, C, codes, off, "pq_smem_f16")
         assert_close(h, ref, tol_16)
         fin = np.isfinite(ref)
-        assert np.abs(h[fin] - ref[fin]).max() > 1e-5 * Nq * max(1.0, dhat_norm)
+        assert np.abs(h[fin] - ref[fin]).max() > 1e-5 * Nq  # several times the plain fp32 bound of north_star
 
 
 def test_f16_table_needs_whole_16_row_slices():
