@@ -79,6 +79,111 @@ topk_level_kernel(const float* __restrict__ scores, const uint64_t* __restrict__
     }
 }
 
+// ---- k <= 128 (the paper's top-100): the same chunk -> `keep` best keys step without sorting the whole chunk ---------
+// A chunk is 32 runs of 128 keys, one run per warp, four keys per thread in registers (logical position p = 4*lane + j).
+//   1. every warp sorts its run with a bitonic network that never leaves the warp: strides 1 and 2 are exchanges between a
+//      thread's own registers, strides 4..64 are shuffles with lane ^ (stride / 4).  Even runs end descending, odd runs
+//      ascending (the network's usual direction rule on the chunk-wide position).
+//   2. five halving steps: run pairs (descending, ascending) are combined position by position with max(), which leaves
+//      a bitonic run holding exactly the 128 largest of the 256 keys; one bitonic merge (again inside the warp) sorts it in
+//      the direction its new run index asks for.  The absorbed run travels through shared memory; every warp writes its
+//      own 1 KB region at most once, so a step costs one __syncthreads and there is no write-after-read hazard.
+// 5 block-wide barriers instead of the 78 of the full sort; keys are unique (the index is part of the key), so the
+// result is the same set in the same order as the sorting kernel's, bit for bit.
+__device__ __forceinline__ void cmpx(uint64_t& a, uint64_t& b, bool desc) {  // a at the lower position
+    const uint64_t lo = a < b ? a : b, hi = a < b ? b : a;
+    a = desc ? hi : lo;
+    b = desc ? lo : hi;
+}
+// one compare-exchange stage of the network at `stride` for this thread's four keys; desc: direction of the stage
+__device__ __forceinline__ void stage(uint64_t (&e)[4], int stride, bool desc, int lane) {
+    if (stride == 1) {
+        cmpx(e[0], e[1], desc);
+        cmpx(e[2], e[3], desc);
+    } else if (stride == 2) {
+        cmpx(e[0], e[2], desc);
+        cmpx(e[1], e[3], desc);
+    } else {
+        const int lm = stride >> 2;
+        const bool lower = (lane & lm) == 0;  // this thread holds the lower position of each pair
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint64_t o = __shfl_xor_sync(0xffffffffu, e[j], lm);
+            const bool take_max = lower == desc;
+            e[j] = take_max ? (e[j] > o ? e[j] : o) : (e[j] < o ? e[j] : o);
+        }
+    }
+}
+
+constexpr int RUN = 128;  // keys per warp; the small-k kernel serves keep <= RUN
+
+__global__ void __launch_bounds__(THREADS)
+topk_level_small_kernel(const float* __restrict__ scores, const uint64_t* __restrict__ keys_in, int64_t n,
+                        int64_t in_pitch, int keep, uint64_t* __restrict__ keys_out, int64_t out_pitch,
+                        float* __restrict__ values, int64_t* __restrict__ indices, int k) {
+    __shared__ uint64_t xch[CHUNK];
+    const int q = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t base = (int64_t)blockIdx.x * CHUNK + warp * RUN;
+    uint64_t e[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {  // any placement will do (the run is sorted next): coalesced rows of 32
+        const int64_t i = base + j * 32 + lane;
+        uint64_t kk = 0;  // below every real key
+        if (i < n) kk = scores ? make_key(scores[(int64_t)q * in_pitch + i], (uint32_t)i) : keys_in[(int64_t)q * in_pitch + i];
+        e[j] = kk;
+    }
+    // 1. sort the run; direction of a stage = the usual (position & size) == 0 on the chunk-wide position warp*128 + p
+#pragma unroll
+    for (int size = 2; size <= RUN; size <<= 1) {
+#pragma unroll
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            // (P & size) == 0 for P = 128*warp + 4*lane + j: size 2 is a register bit, 4..64 a lane bit, 128 the warp's parity
+            if (size == 2) {  // pairs (0,1) descending, (2,3) ascending
+                cmpx(e[0], e[1], true);
+                cmpx(e[2], e[3], false);
+            } else {
+                const bool desc = size == RUN ? (warp & 1) == 0 : (lane & (size >> 2)) == 0;
+                stage(e, stride, desc, lane);
+            }
+        }
+    }
+    // 2. halving steps: warp w absorbs warp w + 2^s
+#pragma unroll
+    for (int s = 0; s < 5; ++s) {
+        const int step = 1 << s;
+        const bool alive = (warp & (step - 1)) == 0;
+        if (alive && (warp & step)) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) xch[warp * RUN + j * 32 + lane] = e[j];
+        }
+        __syncthreads();
+        if (alive && !(warp & step)) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint64_t o = xch[(warp + step) * RUN + j * 32 + lane];
+                e[j] = e[j] > o ? e[j] : o;
+            }
+            const bool desc = ((warp >> (s + 1)) & 1) == 0;  // parity of the new run's index
+#pragma unroll
+            for (int stride = RUN >> 1; stride > 0; stride >>= 1) stage(e, stride, desc, lane);
+        }
+    }
+    if (warp == 0) {  // the chunk's 128 best, descending, at positions p = 4*lane + j
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int p = 4 * lane + j;
+            if (values) {
+                if (p < k) {
+                    values[(int64_t)q * k + p] = key_score(e[j]);
+                    indices[(int64_t)q * k + p] = (int64_t)(uint32_t)(~(uint32_t)e[j]);
+                }
+            } else if (p < keep) {
+                keys_out[(int64_t)q * out_pitch + (int64_t)blockIdx.x * keep + p] = e[j];
+            }
+        }
+    }
+}
+
 int64_t chunks_of(int64_t n) { return (n + CHUNK - 1) / CHUNK; }
 
 constexpr int MAX_SHARDS = 64;
@@ -108,8 +213,9 @@ int run_levels(const float* scores, const uint64_t* keys_in, int64_t n, int64_t 
         const int64_t nch = chunks_of(n);
         const bool last = nch == 1;
         dim3 grid((unsigned)nch, (unsigned)Q);
-        topk_level_kernel<<<grid, THREADS, 0, stream>>>(s_in, k_in, n, in_pitch, k, last ? nullptr : buf[level & 1], pitch1,
-                                                        last ? values : nullptr, last ? indices : nullptr, k);
+        auto* kern = k <= RUN ? topk_level_small_kernel : topk_level_kernel;
+        kern<<<grid, THREADS, 0, stream>>>(s_in, k_in, n, in_pitch, k, last ? nullptr : buf[level & 1], pitch1,
+                                           last ? values : nullptr, last ? indices : nullptr, k);
         count_launch();
         if (cudaGetLastError() != cudaSuccess) return TMS_ERR_CUDA;
         if (last) break;

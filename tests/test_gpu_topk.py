@@ -28,6 +28,18 @@ def test_random_scores(B, k):
     check(rng.standard_normal((3, B)), k)
 
 
+@pytest.mark.parametrize("k", [1, 2, 3, 64, 100, 127, 128, 129])  # k <= 128: the warp-resident kernel; 129: the sorting one
+@pytest.mark.parametrize("B", [130, 4095, 4096, 4097, 50_000, 1_048_577])  # one chunk, chunk edges, two / three levels
+def test_both_level_kernels_around_their_switch_point(B, k):
+    if k > B:
+        pytest.skip("k <= B")
+    rng = np.random.default_rng(1000 * k + B % 997)
+    s = rng.standard_normal((2, B))
+    s[:, rng.integers(0, B, size=B // 5)] = -np.inf   # empty documents
+    s[0, : min(B, 300)] = 1.0                         # a long tie at the top: lower index first
+    check(s, k)
+
+
 def test_ties_and_neg_inf_follow_the_index_rule():
     rng = np.random.default_rng(5)
     s = rng.integers(-2, 3, size=(4, 20_000)).astype(np.float64)  # five distinct values: thousands of ties
