@@ -95,24 +95,29 @@ __device__ __forceinline__ void cmpx(uint64_t& a, uint64_t& b, bool desc) {  // 
     a = desc ? hi : lo;
     b = desc ? lo : hi;
 }
-// one compare-exchange stage of the network at `stride` for this thread's four keys; desc: direction of the stage
-__device__ __forceinline__ void stage(uint64_t (&e)[4], int stride, bool desc, int lane) {
-    if (stride == 1) {
-        cmpx(e[0], e[1], desc);
-        cmpx(e[2], e[3], desc);
-    } else if (stride == 2) {
-        cmpx(e[0], e[2], desc);
-        cmpx(e[1], e[3], desc);
-    } else {
-        const int lm = stride >> 2;
-        const bool lower = (lane & lm) == 0;  // this thread holds the lower position of each pair
+// The network's stages for this thread's four keys (position p = 4*lane + j).  Strides 1 and 2 pair a thread's own
+// registers; a stride >= 4 pairs lane with lane ^ (stride / 4), same register.  desc: direction of the stage.
+__device__ __forceinline__ void stage_regs(uint64_t (&e)[4], bool desc) {  // stride 2, then stride 1
+    cmpx(e[0], e[2], desc);
+    cmpx(e[1], e[3], desc);
+    cmpx(e[0], e[1], desc);
+    cmpx(e[2], e[3], desc);
+}
+__device__ __forceinline__ void stage_lanes(uint64_t (&e)[4], int lm, bool desc, int lane) {
+    const bool take_max = ((lane & lm) == 0) == desc;  // the lower position of a pair keeps the larger key iff descending
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint64_t o = __shfl_xor_sync(0xffffffffu, e[j], lm);
-            const bool take_max = lower == desc;
-            e[j] = take_max ? (e[j] > o ? e[j] : o) : (e[j] < o ? e[j] : o);
-        }
+    for (int j = 0; j < 4; ++j) {
+        const uint64_t o = __shfl_xor_sync(0xffffffffu, e[j], lm);
+        e[j] = take_max ? (e[j] > o ? e[j] : o) : (e[j] < o ? e[j] : o);
     }
+}
+// all stages of one merge of `size` keys (strides size/2 .. 1).  The lane loop is NOT unrolled: the fully unrolled kernel
+// was 40 KB of straight-line code that every one of the 32 warps streamed through once, and ran at the instruction
+// fetch rate (19 us for a single chunk); as loops it is a few KB.
+__device__ __forceinline__ void merge(uint64_t (&e)[4], int size, bool desc, int lane) {
+#pragma unroll 1
+    for (int lm = size >> 3; lm > 0; lm >>= 1) stage_lanes(e, lm, desc, lane);
+    stage_regs(e, desc);
 }
 
 constexpr int RUN = 128;  // keys per warp; the small-k kernel serves keep <= RUN
@@ -132,23 +137,16 @@ topk_level_small_kernel(const float* __restrict__ scores, const uint64_t* __rest
         if (i < n) kk = scores ? make_key(scores[(int64_t)q * in_pitch + i], (uint32_t)i) : keys_in[(int64_t)q * in_pitch + i];
         e[j] = kk;
     }
-    // 1. sort the run; direction of a stage = the usual (position & size) == 0 on the chunk-wide position warp*128 + p
-#pragma unroll
-    for (int size = 2; size <= RUN; size <<= 1) {
-#pragma unroll
-        for (int stride = size >> 1; stride > 0; stride >>= 1) {
-            // (P & size) == 0 for P = 128*warp + 4*lane + j: size 2 is a register bit, 4..64 a lane bit, 128 the warp's parity
-            if (size == 2) {  // pairs (0,1) descending, (2,3) ascending
-                cmpx(e[0], e[1], true);
-                cmpx(e[2], e[3], false);
-            } else {
-                const bool desc = size == RUN ? (warp & 1) == 0 : (lane & (size >> 2)) == 0;
-                stage(e, stride, desc, lane);
-            }
-        }
-    }
+    // 1. sort the run; direction of a merge = the usual (P & size) == 0 on the chunk-wide position P = 128*warp + 4*lane + j:
+    //    size 2 is a register bit, sizes 4..64 a lane bit, 128 the warp's parity
+    cmpx(e[0], e[1], true);   // size 2: pair (0,1) descending, pair (2,3) ascending
+    cmpx(e[2], e[3], false);
+    stage_regs(e, (lane & 1) == 0);  // size 4
+#pragma unroll 1
+    for (int size = 8; size <= RUN; size <<= 1)
+        merge(e, size, size == RUN ? (warp & 1) == 0 : (lane & (size >> 2)) == 0, lane);
     // 2. halving steps: warp w absorbs warp w + 2^s
-#pragma unroll
+#pragma unroll 1
     for (int s = 0; s < 5; ++s) {
         const int step = 1 << s;
         const bool alive = (warp & (step - 1)) == 0;
@@ -163,9 +161,7 @@ topk_level_small_kernel(const float* __restrict__ scores, const uint64_t* __rest
                 const uint64_t o = xch[(warp + step) * RUN + j * 32 + lane];
                 e[j] = e[j] > o ? e[j] : o;
             }
-            const bool desc = ((warp >> (s + 1)) & 1) == 0;  // parity of the new run's index
-#pragma unroll
-            for (int stride = RUN >> 1; stride > 0; stride >>= 1) stage(e, stride, desc, lane);
+            merge(e, RUN, ((warp >> (s + 1)) & 1) == 0, lane);  // direction: parity of the new run's index
         }
     }
     if (warp == 0) {  // the chunk's 128 best, descending, at positions p = 4*lane + j
