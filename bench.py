@@ -386,7 +386,8 @@ def timed_region(wl, steps, warmup, local_rank, sync_all, shard, min_ms=0.0, max
     """W warm-up steps, then exactly K steps with per-step CUDA events on the launching stream; clocks, throttle reasons and
     board power are sampled through NVML while the steps run (samples taken before the first step starts or after the
     last one ends are dropped).  min_ms > 0 (secondary workloads): K is raised until the region lasts about min_ms, so
-    that the 5 ms NVML sampler sees it (at most max_steps).  Returns per-step times and the max-over-ranks total."""
+    that the 5 ms NVML sampler sees it (at most max_steps); a region that still comes out short is timed again with K
+    scaled up.  Returns per-step times and the max-over-ranks total."""
     for _ in range(warmup):
         wl.step()
     sync_all()
@@ -401,6 +402,16 @@ def timed_region(wl, steps, warmup, local_rank, sync_all, shard, min_ms=0.0, max
         sync_all()
         est = max(w0.elapsed_time(w1) / 5, 1e-3)
         steps = int(min(max_steps, max(steps, np.ceil(min_ms / est))))
+    for _attempt in range(3):
+        out = _timed_steps(wl, steps, local_rank, sync_all, shard)
+        region_ms = out[4]
+        if min_ms <= 0 or region_ms >= 0.7 * min_ms or steps >= max_steps:
+            break
+        steps = int(min(max_steps, np.ceil(steps * 1.1 * min_ms / max(region_ms, 1e-3))))
+    return out[:4]
+
+
+def _timed_steps(wl, steps, local_rank, sync_all, shard):
     sampler = ClockSampler(local_rank)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -422,9 +433,10 @@ def timed_region(wl, steps, warmup, local_rank, sync_all, shard, min_ms=0.0, max
     clocks = sampler.stop(t_first, t_last)
     launches = wl.tms.tms_launch_count() - n0
     step_ms = np.array([a.elapsed_time(b) for a, b in ev])
-    total_ms = float(step_ms.sum()) if wl.flush is not None else float(t_start.elapsed_time(t_end))
+    region_ms = float(t_start.elapsed_time(t_end))  # flushes included: what the clock sampler saw
+    total_ms = float(step_ms.sum()) if wl.flush is not None else region_ms
     _, total_ms = shard.aggregate_throughput(1.0, total_ms, wl.dev)  # MAX over ranks of the device-timed region
-    return step_ms, total_ms, clocks, int(launches)
+    return step_ms, total_ms, clocks, int(launches), region_ms
 
 
 def roofline_of(wl, step_ms, total_ms, clocks, peaks):
