@@ -673,8 +673,9 @@ def main():
         rs = roofline_of(wl, s_ms, s_total, s_clk, peaks)
         line["sustained"] = {"steps": int(s_ms.size), "ms_per_step": s_total / s_ms.size,
                              "ms_median": float(np.median(s_ms)), "bound": rs["bound"], "frac_burst": rs["frac"],
-                             "frac_sustained": rs.get("tensor", {}).get("frac_sustained") if rs["bound"] == "tensor"
-                             else None, "hbm_frac": rs["hbm"]["frac"],
+                             "tensor_frac_burst": rs.get("tensor", {}).get("frac_burst"),
+                             "tensor_frac_sustained": rs.get("tensor", {}).get("frac_sustained"),
+                             "hbm_frac": rs["hbm"]["frac"],
                              "sm_mhz": s_clk.get("sm_mhz"), "reasons": s_clk.get("reasons"),
                              "samples": s_clk.get("samples"), "power_w_mean": s_clk.get("power_w_mean")}
     # compact copy of every secondary result, LAST in the line so that a truncated record still carries all of them:
